@@ -1,0 +1,267 @@
+/*
+ * bfly_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * A plain, slow, float64 CPU statement of what the butterfly-filtering hot path
+ * computes: direct time-domain correlation of a data series against chirp
+ * templates, quadrature magnitude over the sliding data norm, maximum over lags
+ * and its lag, and the thresholded time-frequency count map.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may call this.  It shares no code with the CUDA path
+ * (paper_1802_01685_b200/): no common header, helper, table or constant.
+ *
+ * Source of the definition.  PAPER.md prints no formula for the template, rho or
+ * the map (it describes matched filtering against a bank of ~1 s ascending and
+ * descending chirps, PAPER.md:54-62 (sec. 2.1); correlation over a 16-s segment,
+ * PAPER.md:70, 120 (sec. 2.2, Fig. 5 caption); thresholded output).
+ * The formulas are those of BASELINE.json (north_star; configs[0]: "h(t) =
+ * cos/sin(2 pi (f0 t + 1/2 f1 t^2)) for t in [0,1), each unit-L2-normalized ...
+ * rho(tau) = sqrt(c^2+s^2)/||x_tau||"), in the readings C1-C12 listed in
+ * DESIGN.md ("Readings of the paper") and SURVEY.md section 8(c).
+ *
+ * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): P1 Cauchy-Schwarz,
+ * P2 noise-free injection, P3 time reversal, P4 direct vs FFT, P5 scale
+ * invariance, P6 DFT special case against numpy.fft, P7 Parseval sum, P8 noise
+ * expectation 2/L, P9 matched injection in noise, P10 map by brute force,
+ * P11 chunking.  Parity unpinned (fixed by DESIGN.md readings only, the paper
+ * being silent): the choice of map coordinates (C10: time = start of the matched
+ * window, frequency = f0) and the per-chunk hit semantics of streaming (C11).
+ *
+ * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC (oracle/build.py).
+ * -ffp-contract=off and no -ffast-math: every sum below is evaluated in the order
+ * written, in IEEE float64.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define BFO_PI 3.14159265358979323846
+
+/* C1 (BASELINE.json configs[0]): template samples
+ *   t_k = k/fs, phi_k = 2 pi (f0 t_k + 1/2 f1 t_k^2), hc[k] = cos phi_k, hs[k] = sin phi_k,
+ *   k = 0..L-1; phase zero at the first sample; no window. */
+void bfo_template(double fs, int L, double f0, double f1, double *hc, double *hs)
+{
+    for (int k = 0; k < L; ++k) {
+        double t = (double)k / fs;
+        double phi = 2.0 * BFO_PI * (f0 * t + 0.5 * f1 * t * t);
+        hc[k] = cos(phi);
+        hs[k] = sin(phi);
+    }
+}
+
+/* C2 ("each unit-L2-normalized", BASELINE.json configs[0]): the L2 norms of the
+ * cosine and of the sine template, taken separately. */
+void bfo_template_norms(int L, const double *hc, const double *hs, double *nc, double *ns)
+{
+    double a = 0.0, b = 0.0;
+    for (int k = 0; k < L; ++k) {
+        a += hc[k] * hc[k];
+        b += hs[k] * hs[k];
+    }
+    *nc = sqrt(a);
+    *ns = sqrt(b);
+}
+
+/* The literal definition at one (template, lag) (SURVEY.md section 8(c) pseudo-code):
+ *   c  = sum_k x[tau+k] hc[k] / nc   (0 if nc == 0)           C2, C4
+ *   s  = sum_k x[tau+k] hs[k] / ns   (0 if ns == 0)
+ *   n2 = sum_k x[tau+k]^2                                      C6
+ *   rho = n2 > 0 ? sqrt(c^2 + s^2) / sqrt(n2) : 0              C6, C7
+ * Optionally returns the two normalised components c/||x_tau|| and s/||x_tau||.
+ * x is the fp32 input, upcast (C12). */
+double bfo_rho_at(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
+                  int64_t tau, double *c_over_norm, double *s_over_norm)
+{
+    (void)n_samples;
+    double *hc = (double *)malloc(sizeof(double) * (size_t)L);
+    double *hs = (double *)malloc(sizeof(double) * (size_t)L);
+    double nc, ns;
+    bfo_template(fs, L, f0, f1, hc, hs);
+    bfo_template_norms(L, hc, hs, &nc, &ns);
+    double c = 0.0, s = 0.0, n2 = 0.0;
+    for (int k = 0; k < L; ++k) {
+        double xv = (double)x[tau + k];
+        c += xv * hc[k];
+        s += xv * hs[k];
+        n2 += xv * xv;
+    }
+    c = (nc > 0.0) ? c / nc : 0.0;
+    s = (ns > 0.0) ? s / ns : 0.0;
+    double rho = 0.0, cn = 0.0, sn = 0.0;
+    if (n2 > 0.0) {
+        double nx = sqrt(n2);
+        rho = sqrt(c * c + s * s) / nx;
+        cn = c / nx;
+        sn = s / nx;
+    }
+    if (c_over_norm) *c_over_norm = cn;
+    if (s_over_norm) *s_over_norm = sn;
+    free(hc);
+    free(hs);
+    return rho;
+}
+
+/* C6: sliding squared norm n2[tau] = sum_k x[tau+k]^2, each lag summed on its own
+ * (no running-sum update), for lag_begin <= tau < lag_end. */
+void bfo_sliding_n2(const float *x, int L, int64_t lag_begin, int64_t lag_end, double *n2)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t tau = lag_begin; tau < lag_end; ++tau) {
+        double a = 0.0;
+        for (int k = 0; k < L; ++k) {
+            double xv = (double)x[tau + k];
+            a += xv * xv;
+        }
+        n2[tau - lag_begin] = a;
+    }
+}
+
+/* Sums over k for a run of lags at once.  For every lag the sum over k is
+ * accumulated in ascending k exactly as in bfo_rho_at (the loops over k and over
+ * the lags of the run are interchanged so that the compiler can vectorise across
+ * lags; no sum is re-associated; tests check bit-equality with bfo_rho_at). */
+#define BFO_RUN 1024
+static void bfo_dots_run(const double *restrict xd, int L, const double *restrict hc,
+                         const double *restrict hs,
+                         int64_t tau0, int n, double *restrict c, double *restrict s)
+{
+    for (int i = 0; i < n; ++i) { c[i] = 0.0; s[i] = 0.0; }
+    for (int k = 0; k < L; ++k) {
+        const double a = hc[k], b = hs[k];
+        const double *xp = xd + tau0 + k;
+        for (int i = 0; i < n; ++i) {
+            c[i] += xp[i] * a;
+            s[i] += xp[i] * b;
+        }
+    }
+}
+
+/* rho_j(tau) of ONE template for lag_begin <= tau < lag_end (needed for the argmax
+ * rule and the pins).  c_out / s_out (optional) receive c/||x_tau||, s/||x_tau||. */
+void bfo_rho_series(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
+                    int64_t lag_begin, int64_t lag_end, double *rho, double *c_out, double *s_out)
+{
+    double *xd = (double *)malloc(sizeof(double) * (size_t)n_samples);
+    for (int64_t i = 0; i < n_samples; ++i) xd[i] = (double)x[i];
+    double *hc = (double *)malloc(sizeof(double) * (size_t)L);
+    double *hs = (double *)malloc(sizeof(double) * (size_t)L);
+    double nc, ns;
+    bfo_template(fs, L, f0, f1, hc, hs);
+    bfo_template_norms(L, hc, hs, &nc, &ns);
+    double c[BFO_RUN], s[BFO_RUN];
+    for (int64_t tau0 = lag_begin; tau0 < lag_end; tau0 += BFO_RUN) {
+        int n = (int)((lag_end - tau0 < BFO_RUN) ? (lag_end - tau0) : BFO_RUN);
+        bfo_dots_run(xd, L, hc, hs, tau0, n, c, s);
+        for (int i = 0; i < n; ++i) {
+            double n2 = 0.0;
+            for (int k = 0; k < L; ++k) n2 += xd[tau0 + i + k] * xd[tau0 + i + k];
+            double cv = (nc > 0.0) ? c[i] / nc : 0.0;
+            double sv = (ns > 0.0) ? s[i] / ns : 0.0;
+            double r = 0.0, cn = 0.0, sn = 0.0;
+            if (n2 > 0.0) {
+                double nx = sqrt(n2);
+                r = sqrt(cv * cv + sv * sv) / nx;
+                cn = cv / nx;
+                sn = sv / nx;
+            }
+            rho[tau0 - lag_begin + i] = r;
+            if (c_out) c_out[tau0 - lag_begin + i] = cn;
+            if (s_out) s_out[tau0 - lag_begin + i] = sn;
+        }
+    }
+    free(hc); free(hs); free(xd);
+}
+
+/* The whole search (SURVEY.md section 8(c) pseudo-code; north_star): for each template
+ * j, rho_max[j] = max over lag_begin <= tau < lag_end of rho_j(tau) and arg_lag[j] =
+ * the smallest tau attaining it (strict '>' while scanning upwards, C8).  Valid
+ * lags only (C5): requires 0 <= lag_begin <= lag_end <= n_samples - L + 1.
+ * Templates are independent; OpenMP runs them on n_threads threads (0 = default).
+ * Returns the number of threads used, or -1 on bad arguments. */
+int bfo_correlate(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
+                  const double *f0, const double *f1, int64_t lag_begin, int64_t lag_end,
+                  double *rho_max, int32_t *arg_lag, int n_threads)
+{
+    if (L < 1 || n_samples < L || lag_begin < 0 || lag_end < lag_begin ||
+        lag_end > n_samples - L + 1)
+        return -1;
+    const int64_t n_lags = lag_end - lag_begin;
+    double *xd = (double *)malloc(sizeof(double) * (size_t)n_samples);
+    for (int64_t i = 0; i < n_samples; ++i) xd[i] = (double)x[i];
+    double *n2 = (double *)malloc(sizeof(double) * (size_t)(n_lags > 0 ? n_lags : 1));
+    bfo_sliding_n2(x, L, lag_begin, lag_end, n2);
+    int used = 1;
+#ifdef _OPENMP
+    if (n_threads <= 0) n_threads = omp_get_max_threads();
+    used = n_threads;
+#else
+    n_threads = 1;
+#endif
+#pragma omp parallel num_threads(n_threads)
+    {
+        double *hc = (double *)malloc(sizeof(double) * (size_t)L);
+        double *hs = (double *)malloc(sizeof(double) * (size_t)L);
+        double c[BFO_RUN], s[BFO_RUN];
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t j = 0; j < n_templates; ++j) {
+            double nc, ns;
+            bfo_template(fs, L, f0[j], f1[j], hc, hs);
+            bfo_template_norms(L, hc, hs, &nc, &ns);
+            double best = -1.0;
+            int64_t arg = lag_begin;
+            for (int64_t tau0 = lag_begin; tau0 < lag_end; tau0 += BFO_RUN) {
+                int n = (int)((lag_end - tau0 < BFO_RUN) ? (lag_end - tau0) : BFO_RUN);
+                bfo_dots_run(xd, L, hc, hs, tau0, n, c, s);
+                for (int i = 0; i < n; ++i) {
+                    double cv = (nc > 0.0) ? c[i] / nc : 0.0;
+                    double sv = (ns > 0.0) ? s[i] / ns : 0.0;
+                    double nn = n2[tau0 - lag_begin + i];
+                    double r = (nn > 0.0) ? sqrt(cv * cv + sv * sv) / sqrt(nn) : 0.0;
+                    if (r > best) { best = r; arg = tau0 + i; }
+                }
+            }
+            if (n_lags == 0) best = 0.0;
+            rho_max[j] = best;
+            arg_lag[j] = (int32_t)arg;
+        }
+        free(hc); free(hs);
+    }
+    free(n2); free(xd);
+    return used;
+}
+
+/* Threshold and map (C9, C10; "rho exceeding kappa sigma", PAPER.md:54
+ * "chirp-based spectrograms"): for each template with rho_max[j] > kappa (strict),
+ *   tbin = (lag_origin + arg_lag[j]) / samples_per_tbin   (integer division)
+ *   fbin = floor((f0[j] - f_lo) / df)
+ * and map[tbin][fbin] += 1 if the bin is inside the map.  counters[0] counts all
+ * hits, counters[1] the hits that fell outside.  map is accumulated into. */
+void bfo_map(int64_t n_templates, const double *f0, const double *rho_max, const int32_t *arg_lag,
+             double kappa, int64_t lag_origin, int32_t samples_per_tbin, double f_lo, double df,
+             int32_t n_fbins, int32_t n_tbins, uint32_t *map, uint64_t *counters)
+{
+    for (int64_t j = 0; j < n_templates; ++j) {
+        if (!(rho_max[j] > kappa)) continue;
+        counters[0] += 1;
+        int64_t tbin = (lag_origin + (int64_t)arg_lag[j]) / samples_per_tbin;
+        double fb = floor((f0[j] - f_lo) / df);
+        if (tbin >= 0 && tbin < n_tbins && fb >= 0.0 && fb < (double)n_fbins)
+            map[tbin * (int64_t)n_fbins + (int64_t)fb] += 1;
+        else
+            counters[1] += 1;
+    }
+}
+
+int bfo_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
