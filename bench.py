@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the butterfly-filtering hot path on B200.
+
+A step = one pass of the whole hot path (rows A2-A8: sliding norm, data spectra, correlation
+core with fused epilogue, threshold + map) of one data segment against the whole template
+bank.  Default workload = BASELINE.json configs[3], "Paper-scale bank": 2^23 templates of
+L = 4096 against a 16-s segment (65536 samples at 4096 Hz), i.e. exactly the paper's unit:
+one correlation = one template x one 16-s segment over all 61441 lags.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  With N > 1 (torchrun) every rank runs the same job on its own
+GPU (replicas only, no collective on the data path); value = all
+ranks' correlations / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import bank_grid, default_map_grid, get_config, make_data, sub_bank_indices  # noqa: E402
+
+METRIC = "1-s template correlations/sec"
+UNIT = "correlations/s"
+REF_LAGS = 61441            # lags of one paper-unit correlation (16 s at 4096 Hz, L = 4096)
+FFT_B = 8192                # overlap-save block of the FFT form
+SM_COUNT, FP32_LANES = 148, 128
+
+
+def correlations_per_step(cfg, n_templates):
+    """Paper-unit correlations in one step: templates x lags / 61441 (= templates at config 4)."""
+    return n_templates * cfg.n_lags / REF_LAGS
+
+
+def fft_form_flops(cfg, n_templates):
+    """Algorithmic flops of one launch of the FFT-form core: per template
+    one template FFT + per block one spectral multiply (6 B) and one inverse FFT, each FFT
+    counted 5 B log2 B."""
+    V = FFT_B - cfg.L + 1
+    n_blocks = (cfg.n_lags + V - 1) // V
+    fft = 5 * FFT_B * int(math.log2(FFT_B))
+    return n_templates * ((n_blocks + 1) * fft + n_blocks * 6 * FFT_B)
+
+
+def direct_form_flops(cfg, n_templates):
+    return n_templates * 2 * (2 * cfg.L * cfg.n_lags)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def time_oracle(cfg, x, f0, f1, seconds):
+    """The oracle as it stands on the host cores, on a bounded sample of the workload: as many
+    of the given templates (all lags) as fit in about `seconds`.  Returns (corr/s, n, s, cores)."""
+    import oracle
+    n0 = min(8, len(f0))
+    t = time.perf_counter()
+    oracle.correlate(x, cfg.fs_hz, cfg.L, f0[:n0], f1[:n0])
+    dt0 = time.perf_counter() - t
+    n = int(max(n0, min(len(f0), (seconds / max(dt0, 1e-3)) * n0)))
+    t = time.perf_counter()
+    oracle.correlate(x, cfg.fs_hz, cfg.L, f0[:n], f1[:n])
+    dt = time.perf_counter() - t
+    return correlations_per_step(cfg, n) / dt, n, dt, oracle.max_threads()
+
+
+def run_reference(args, cfg, rank):
+    """--impl reference: the float64 oracle on the box's host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    x = make_data(cfg)
+    f0a, f1a = bank_grid(cfg)
+    idx = sub_bank_indices(cfg, 4096, seed=7, halfwidth=0, max_track=0)
+    f0, f1 = f0a[idx], f1a[idx]
+    # size one step at about 8 s of CPU work
+    t = time.perf_counter()
+    oracle.correlate(x, cfg.fs_hz, cfg.L, f0[:8], f1[:8])
+    per8 = time.perf_counter() - t
+    n = int(max(8, min(len(f0) // max(args.steps + args.warmup, 1), 8.0 / max(per8, 1e-3) * 8)))
+    pos = 0
+    for _ in range(args.warmup):
+        oracle.correlate(x, cfg.fs_hz, cfg.L, f0[pos:pos + n], f1[pos:pos + n]); pos += n
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.correlate(x, cfg.fs_hz, cfg.L, f0[pos:pos + n], f1[pos:pos + n]); pos += n
+    dt = time.perf_counter() - t
+    value = correlations_per_step(cfg, n) * args.steps / dt
+    sample = f"{n} templates x all {cfg.n_lags} lags per step, seeded stratified sample of the bank"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {cfg.index} ({cfg.name})", "templates_per_step": n,
+                   "n_samples": cfg.n_samples, "L": cfg.L, "lags": cfg.n_lags},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(),
+                         "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config, 1-based")
+    ap.add_argument("--form", type=int, default=0, help="0 default (FFT), 1 FFT, 2 direct")
+    ap.add_argument("--templates", type=int, default=0,
+                    help="development only: first n templates of the bank (not a bench line)")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = get_config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1802_01685_b200 as bfly
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    # ---- inputs (seeded, synthetic) and the persistent bank (A1)
+    x = make_data(cfg)
+    t0 = time.perf_counter()
+    if args.templates:
+        f0a, f1a = bank_grid(cfg)
+        bank = bfly.make_bank(cfg.fs_hz, cfg.L, f0a[:args.templates], f1a[:args.templates], local)
+    else:
+        bank = bfly.make_bank_grid(cfg.fs_hz, cfg.L, cfg.f0_lo, cfg.f0_hi, cfg.n_f0,
+                                   cfg.f1_lo, cfg.f1_hi, cfg.n_f1, local)
+    bank_s = time.perf_counter() - t0
+    T = len(bank)
+    bank.reserve(cfg.n_samples)
+    grid = default_map_grid(cfg)
+    dev = torch.device("cuda", local)
+    xd = torch.from_numpy(x).to(dev)
+    rho = torch.empty(T, dtype=torch.float32, device=dev)
+    arg = torch.empty(T, dtype=torch.int32, device=dev)
+    m = torch.zeros((grid["n_tbins"], grid["n_fbins"]), dtype=torch.int32, device=dev)
+    cnt = torch.zeros(2, dtype=torch.int64, device=dev)
+    form = args.form
+    chunk = cfg.chunk_samples if cfg.streaming else 0
+
+    def step():
+        if cfg.streaming:
+            raise SystemExit("config 5 is a parity-test case; bench on configs 1-4")
+        bfly.correlate_form(bank, form, xd, 0, None, rho, arg)
+        bfly.butterfly_map(bank, rho, arg, cfg.kappa, 0, **grid, map_out=m, counters=cnt)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    m.zero_(); cnt.zero_()
+    bank.set_timing(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier(); torch.cuda.synchronize()
+    launches0 = bfly.launch_count()
+    core_ms = []
+    e0.record()
+    for _ in range(args.steps):
+        step()
+        core_ms.append(bank.core_ms())       # waits for this step's core kernel only
+    e1.record()
+    torch.cuda.synchronize(); barrier()
+    launches = bfly.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    bank.set_timing(False)
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        tms = torch.tensor([ms], device=dev)
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        ms = float(tms.item())
+    corr_step = correlations_per_step(cfg, T)
+    value = world * corr_step * args.steps / (ms * 1e-3)
+
+    # ---- e2e: the same step through bfly_search_host with HOST buffers (copies inside)
+    e2e = None
+    if not args.no_e2e:
+        xh = torch.from_numpy(x).pin_memory()
+        bfly.search_host(bank, xh, chunk, cfg.kappa, **grid)          # warm-up (allocations)
+        barrier(); torch.cuda.synchronize()
+        t = time.perf_counter()
+        for _ in range(args.steps):
+            bfly.search_host(bank, xh, chunk, cfg.kappa, **grid)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t
+        if world > 1:
+            tdt = torch.tensor([dt], device=dev)
+            dist.all_reduce(tdt, op=dist.ReduceOp.MAX)
+            dt = float(tdt.item())
+        e2e = {"value": world * corr_step * args.steps / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(x.nbytes),
+               "d2h_bytes_per_step": int(T * 8 + m.numel() * 4 + 16)}
+
+    if rank == 0:
+        # ---- roofline of the dominant kernel (the correlation core), timed live above
+        core_s = float(np.mean(core_ms)) * 1e-3
+        is_fft = form in (0, 1)
+        flops = fft_form_flops(cfg, T) if is_fft else direct_form_flops(cfg, T)
+        peak_tflops = SM_COUNT * FP32_LANES * 2 * 1.965e9 / 1e12
+        achieved = flops / core_s / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get("fft_core_bytes_per_launch" if is_fft
+                                                 else "direct_core_bytes_per_launch")
+        roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                    "frac": achieved / peak_tflops, "traffic": traffic,
+                    "kernel": "fft_correlate_kernel" if is_fft else "direct_kernel",
+                    "kernel_ms": core_s * 1e3, "kernel_share_of_step": core_s * 1e3 * args.steps / ms,
+                    "flops_per_launch": flops,
+                    "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz"}
+        # ---- the oracle beside it, on this box's host cores, on a bounded sample
+        f0a, f1a = bank_grid(cfg)
+        idx = sub_bank_indices(cfg, 1024, seed=7, halfwidth=0, max_track=0)
+        cv, cn, cs, cores = time_oracle(cfg, x, f0a[idx], f1a[idx], args.cpu_seconds)
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"config {cfg.index} ({cfg.name})", "templates": T,
+                       "n_samples": cfg.n_samples, "L": cfg.L, "lags": cfg.n_lags,
+                       "form": "fft" if is_fft else "direct",
+                       "l2": "inputs larger than L2 (bank parameters + outputs "
+                             f"{(T * 48) >> 20} MiB per step)",
+                       "parallelism": "replicas" if world > 1 else "single GPU",
+                       "bank_build_s": bank_s,
+                       "partial_bank_dev_run": bool(args.templates)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline,
+            "pairs_per_s": world * T * cfg.n_lags * args.steps / (ms * 1e-3),
+            "direct_equiv_mac_per_s": world * T * cfg.n_lags * 2 * cfg.L * args.steps / (ms * 1e-3),
+            "cpu_baseline": {"value": cv, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{cn} templates x all {cfg.n_lags} lags of config "
+                                       f"{cfg.index} in {cs:.1f} s (float64 direct)"},
+        }
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

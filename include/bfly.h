@@ -1,0 +1,162 @@
+/*
+ * bfly.h -- C ABI of the B200 (sm_100a) butterfly-filtering search library.
+ *
+ * The hot path of arXiv:1802.01685 sec. 2 ("Deep searches by butterfly filtering"):
+ * correlate a whitened time series against a bank of up to ~8 million 1-second chirp
+ * templates (start frequency f0, frequency derivative f1, ascending and descending;
+ * PAPER.md:54-62) over every time lag (one correlation = one template
+ * against one 16-s segment), keep per template the maximum over lags of the quadrature
+ * correlation magnitude normalised by the sliding data norm and the lag where it falls,
+ * and count the templates exceeding a threshold kappa into a time-frequency "butterfly"
+ * map ("chirp-based spectrograms"; "only tails of butterfly
+ * output rho exceeding kappa sigma are communicated").  The formulas are those of
+ * BASELINE.json (north_star, configs[0]) in the readings listed in DESIGN.md.
+ *
+ *   phi_k    = 2 pi (f0 k/fs + 1/2 f1 (k/fs)^2),              k = 0 .. L-1
+ *   c_j(tau) = sum_k x[tau+k] cos(phi_k) / ||cos phi||_2
+ *   s_j(tau) = sum_k x[tau+k] sin(phi_k) / ||sin phi||_2
+ *   rho_j(tau) = sqrt(c^2 + s^2) / sqrt(sum_k x[tau+k]^2)      (0 where the window is all zero)
+ *   rho_max[j] = max_tau rho_j(tau),  arg_lag[j] = smallest tau attaining it
+ *
+ * Conventions
+ *  - Plain C.  No exceptions, no aborts, nothing is printed.  Every call returns a status
+ *    (BFLY_OK = 0, negative = error); bfly_strerror() names it and bfly_last_error() gives a
+ *    thread-local detail string (e.g. the CUDA error text).
+ *  - "DEVICE" pointers are CUDA device pointers on the bank's device; "HOST" pointers are
+ *    ordinary host memory.  The caller owns every buffer it passes in; the library owns only
+ *    the bank and the workspace inside it (released by bfly_free_bank).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls that
+ *    take a stream are asynchronous: they enqueue work and return; kernel faults surface as
+ *    BFLY_ECUDA at a later call or at the caller's synchronisation.
+ *  - Invalid arguments return BFLY_EINVAL before anything is launched.
+ *  - There is no CPU fallback: on a machine without an sm_100 device every call that needs the
+ *    GPU returns BFLY_EUNSUPPORTED or BFLY_ECUDA.
+ */
+#ifndef BFLY_H
+#define BFLY_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bfly_bank bfly_bank; /* opaque; device-resident; owned by the library */
+
+enum {
+    BFLY_OK = 0,
+    BFLY_EINVAL = -1,       /* bad argument */
+    BFLY_ENOMEM = -2,       /* host or device allocation failed */
+    BFLY_ECUDA = -3,        /* a CUDA runtime call failed; see bfly_last_error() */
+    BFLY_EUNSUPPORTED = -4, /* device is not compute capability 10.x, or form unsupported */
+    BFLY_ERANGE = -5        /* a size exceeds what the library supports (see each call) */
+};
+
+/* Correlation forms (the core, row A4 of DESIGN.md).  All produce the same quantities. */
+enum {
+    BFLY_FORM_DEFAULT = 0, /* the form bfly_correlate() uses: BFLY_FORM_FFT */
+    BFLY_FORM_FFT = 1,     /* hand-written batched overlap-save FFT correlate (fp32) */
+    BFLY_FORM_DIRECT = 2   /* fp32 CUDA-core time-domain sums; slow cross-check of the core */
+};
+
+const char *bfly_strerror(int status);
+const char *bfly_last_error(void);
+
+/* ---- A1: the bank (a persistent bank of chirp templates) -------------
+ * Explicit list of templates.  f0_hz / f1_hzps: HOST pointers, n_templates float64 each (Hz,
+ * Hz/s; any finite values: templates that sweep through 0 Hz or beyond fs/2 are legal, the
+ * definition is the sampled formula).  L = template length in samples (2 <= L <= 4096; the
+ * "1 s" is L/fs).  Computes per template, on the device in float64, 1/||cos phi||^2 and
+ * 1/||sin phi||^2 (0 if the norm is 0) and the fixed-point phase constants used to synthesise
+ * the template inside the correlation kernels; template waveforms are never stored.
+ * Synchronous (returns when the bank is ready).  *out_bank is written only on success. */
+int bfly_make_bank(double fs_hz, int32_t L, int64_t n_templates,
+                   const double *f0_hz, const double *f1_hzps,
+                   int device, bfly_bank **out_bank);
+
+/* Convenience: inclusive uniform grids f0 = f0_lo + i (f0_hi - f0_lo)/(n_f0 - 1) (likewise
+ * f1), evaluated in float64 exactly like numpy.linspace; template j = i_f0 * n_f1 + i_f1. */
+int bfly_make_bank_grid(double fs_hz, int32_t L,
+                        double f0_lo, double f0_hi, int32_t n_f0,
+                        double f1_lo, double f1_hi, int32_t n_f1,
+                        int device, bfly_bank **out_bank);
+
+void bfly_free_bank(bfly_bank *bank);            /* NULL is allowed */
+int64_t bfly_bank_size(const bfly_bank *bank);   /* number of templates; -1 if bank is NULL */
+
+/* Copy bank parameters of templates [first, first + count) to HOST arrays (any may be NULL):
+ * f0, f1 (float64) and the stored 1/||cos phi||^2, 1/||sin phi||^2 (float32).  Synchronous. */
+int bfly_bank_get(const bfly_bank *bank, int64_t first, int64_t count,
+                  double *f0_hz, double *f1_hzps, float *inv_nc2, float *inv_ns2);
+
+/* Pre-size the workspace inside the bank for segments of up to max_n_samples samples, so that
+ * later bfly_correlate calls allocate nothing.  Without it the first call with a longer segment
+ * grows the workspace (a synchronising cudaMalloc).  Synchronous. */
+int bfly_bank_reserve(bfly_bank *bank, int64_t max_n_samples);
+
+/* ---- A2-A7: correlate one segment against the whole bank ---------------------------------
+ * x_dev: DEVICE, n_samples fp32, read-only.  Lags searched: lag_begin <= tau < lag_end, which
+ * must lie within the valid lags [0, n_samples - L + 1) (no zero padding, no circular wrap).
+ * rho_max_dev[T] fp32 and arg_lag_dev[T] int32: DEVICE, overwritten; arg_lag is relative to
+ * x_dev[0].  An empty lag range gives rho_max = 0, arg_lag = lag_begin.  n_samples < 2^31.
+ * Asynchronous on `stream`; no host synchronisation; no allocation if the workspace is
+ * already large enough (see bfly_bank_reserve).  One call at a time per bank (the workspace
+ * is shared). */
+int bfly_correlate(const bfly_bank *bank, const float *x_dev, int64_t n_samples,
+                   int64_t lag_begin, int64_t lag_end,
+                   float *rho_max_dev, int32_t *arg_lag_dev, void *stream);
+
+/* The same with an explicit correlation form (BFLY_FORM_*). */
+int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int64_t n_samples,
+                        int64_t lag_begin, int64_t lag_end,
+                        float *rho_max_dev, int32_t *arg_lag_dev, void *stream);
+
+/* ---- A8: threshold and accumulate into the butterfly map ---------------------------------
+ * For every template with rho_max > kappa (strict, compared in fp32):
+ *     tbin = (lag_origin + arg_lag) / samples_per_tbin        (integer division)
+ *     fbin = floor((f0 - f_lo_hz) / df_hz)                    (float64)
+ *     map_dev[tbin * n_fbins + fbin] += 1     if 0 <= tbin < n_tbins and 0 <= fbin < n_fbins
+ * counters_dev[0] += number of hits, counters_dev[1] += hits that fell outside the map.
+ * map_dev (uint32, row-major [n_tbins][n_fbins]) and counters_dev (2 x uint64) are DEVICE
+ * buffers that are ACCUMULATED into (the caller zeroes them).  rho_max_dev / arg_lag_dev are
+ * the outputs of bfly_correlate for the same bank.  lag_origin >= 0 is the absolute sample
+ * index of x_dev[0] in a longer stream (0 for a single segment).  Asynchronous on `stream`. */
+int bfly_butterfly_map(const bfly_bank *bank,
+                       const float *rho_max_dev, const int32_t *arg_lag_dev,
+                       float kappa, int64_t lag_origin, int32_t samples_per_tbin,
+                       double f_lo_hz, double df_hz, int32_t n_fbins, int32_t n_tbins,
+                       uint32_t *map_dev, uint64_t *counters_dev, void *stream);
+
+/* ---- A9 / end-to-end: the whole path on a HOST series ------------------------------------
+ * Runs A2-A8 over a HOST series x_host[n_samples] (fp32), cut into chunks of chunk_samples
+ * samples with an overlap of L samples (hop = chunk_samples - L): chunk c starts at sample
+ * c * hop, searches its local lags [0, hop), the last chunk all the valid lags it has left,
+ * so every valid lag of the series is searched exactly once; lag_origin = c * hop; the map
+ * accumulates over chunks (one hit per template per chunk at most).  chunk_samples <= 0 or
+ * >= n_samples means a single chunk.  Copies each chunk host->device, runs bfly_correlate and
+ * bfly_butterfly_map on `stream`, and at the end copies to the HOST outputs (any may be NULL):
+ * rho_max_host[T] / arg_lag_host[T] of the LAST chunk (arg_lag local to that chunk), map_host
+ * [n_tbins * n_fbins] (overwritten with the run's counts) and counters_host[2].  Synchronous:
+ * returns when the outputs are in host memory. */
+int bfly_search_host(bfly_bank *bank, const float *x_host, int64_t n_samples,
+                     int64_t chunk_samples, float kappa, int32_t samples_per_tbin,
+                     double f_lo_hz, double df_hz, int32_t n_fbins, int32_t n_tbins,
+                     float *rho_max_host, int32_t *arg_lag_host,
+                     uint32_t *map_host, uint64_t *counters_host, void *stream);
+
+/* Measurement aid (bench.py's roofline figure).  With timing enabled, bfly_correlate records a
+ * CUDA event on `stream` immediately before and after the launch of its correlation-core
+ * kernel (row A4-A7; the dominant kernel).  bfly_bank_core_ms waits for the stop event of the
+ * most recent bfly_correlate call on this bank and returns the elapsed device time between the
+ * two events in milliseconds (BFLY_EINVAL if timing is off or no call was made). */
+int bfly_bank_set_timing(bfly_bank *bank, int enable);
+int bfly_bank_core_ms(bfly_bank *bank, float *ms_out);
+
+/* Number of kernel launches the library has enqueued so far in this process (for bench.py's
+ * gpu_launches claim). */
+int64_t bfly_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BFLY_H */

@@ -20,8 +20,10 @@ def chunk_plan(n_samples: int, L: int, chunk: int):
     exactly the valid lags 0 .. n_samples - L."""
     if chunk <= L:
         raise ValueError("chunk must exceed L")
-    H = chunk - L
     total = n_samples - L + 1
+    if chunk >= n_samples:                 # a single chunk takes every valid lag
+        return [(0, n_samples, 0, total)]
+    H = chunk - L
     plan, start = [], 0
     while start < total:
         n = min(chunk, n_samples - start)

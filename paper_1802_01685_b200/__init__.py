@@ -1,0 +1,238 @@
+"""Thin Python binding of libbfly (include/bfly.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used here
+for device memory and streams only.  The functions carry the C names without the `bfly_`
+prefix.  There is no CPU fallback: if the shared library cannot be loaded the import fails,
+and every call that returns a negative status raises BflyError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+__all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
+           "butterfly_map", "search_host", "launch_count", "lib_path",
+           "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT"]
+
+FORM_DEFAULT, FORM_FFT, FORM_DIRECT = 0, 1, 2
+
+
+class BflyError(RuntimeError):
+    def __init__(self, status: int, what: str, detail: str):
+        super().__init__(f"{what}: {detail} (status {status})")
+        self.status = status
+
+
+def _load():
+    path = _build.LIB
+    if _build.is_stale():
+        # Build in-tree when the sources are newer (needs nvcc; works without a GPU).
+        path = _build.build()
+    lib = C.CDLL(path)
+    vp, i32, i64, f64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_float
+    lib.bfly_strerror.restype = C.c_char_p
+    lib.bfly_strerror.argtypes = [C.c_int]
+    lib.bfly_last_error.restype = C.c_char_p
+    lib.bfly_last_error.argtypes = []
+    lib.bfly_make_bank.argtypes = [f64, i32, i64, vp, vp, C.c_int, C.POINTER(vp)]
+    lib.bfly_make_bank_grid.argtypes = [f64, i32, f64, f64, i32, f64, f64, i32, C.c_int,
+                                        C.POINTER(vp)]
+    lib.bfly_free_bank.argtypes = [vp]
+    lib.bfly_free_bank.restype = None
+    lib.bfly_bank_size.argtypes = [vp]
+    lib.bfly_bank_size.restype = i64
+    lib.bfly_bank_get.argtypes = [vp, i64, i64, vp, vp, vp, vp]
+    lib.bfly_bank_reserve.argtypes = [vp, i64]
+    lib.bfly_correlate.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
+    lib.bfly_correlate_form.argtypes = [vp, C.c_int, vp, i64, i64, i64, vp, vp, vp]
+    lib.bfly_butterfly_map.argtypes = [vp, vp, vp, f32, i64, i32, f64, f64, i32, i32, vp, vp, vp]
+    lib.bfly_search_host.argtypes = [vp, vp, i64, i64, f32, i32, f64, f64, i32, i32,
+                                     vp, vp, vp, vp, vp]
+    lib.bfly_bank_set_timing.argtypes = [vp, C.c_int]
+    lib.bfly_bank_core_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    lib.bfly_launch_count.argtypes = []
+    lib.bfly_launch_count.restype = i64
+    for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
+                 "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
+                 "bfly_search_host"):
+        getattr(lib, name).restype = C.c_int
+    return lib, path
+
+
+_lib, _lib_path = _load()
+
+
+def lib_path() -> str:
+    return _lib_path
+
+
+def _check(status: int, what: str):
+    if status != 0:
+        raise BflyError(status, what, (_lib.bfly_last_error() or b"").decode() or
+                        _lib.bfly_strerror(status).decode())
+
+
+def _dev(t: torch.Tensor, dtype, name: str, device=None, numel=None):
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be contiguous {dtype}")
+    if device is not None and t.device.index != device:
+        raise ValueError(f"{name} is on cuda:{t.device.index}, the bank on cuda:{device}")
+    if numel is not None and t.numel() < numel:
+        raise ValueError(f"{name} has {t.numel()} elements, needs {numel}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(device: int):
+    return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+class Bank:
+    """Owner of a bfly_bank handle (device-resident bank parameters and workspace)."""
+
+    def __init__(self, handle, device: int, fs_hz: float, L: int):
+        self._h = handle
+        self.device = device
+        self.fs_hz = float(fs_hz)
+        self.L = int(L)
+
+    def __len__(self):
+        return int(_lib.bfly_bank_size(self._h))
+
+    def close(self):
+        if self._h is not None:
+            _lib.bfly_free_bank(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def get(self, first: int = 0, count: int | None = None):
+        """(f0, f1, 1/||cos||^2, 1/||sin||^2) of templates [first, first+count) as numpy."""
+        count = len(self) - first if count is None else count
+        f0 = np.empty(count, np.float64)
+        f1 = np.empty(count, np.float64)
+        a = np.empty(count, np.float32)
+        b = np.empty(count, np.float32)
+        _check(_lib.bfly_bank_get(self._h, first, count, f0.ctypes.data, f1.ctypes.data,
+                                  a.ctypes.data, b.ctypes.data), "bfly_bank_get")
+        return f0, f1, a, b
+
+    def set_timing(self, enable: bool):
+        _check(_lib.bfly_bank_set_timing(self._h, int(bool(enable))), "bfly_bank_set_timing")
+
+    def core_ms(self) -> float:
+        """Device time of the correlation-core kernel of the last correlate call (ms)."""
+        ms = C.c_float()
+        _check(_lib.bfly_bank_core_ms(self._h, C.byref(ms)), "bfly_bank_core_ms")
+        return float(ms.value)
+
+    def reserve(self, max_n_samples: int):
+        _check(_lib.bfly_bank_reserve(self._h, int(max_n_samples)), "bfly_bank_reserve")
+
+
+def make_bank(fs_hz: float, L: int, f0_hz, f1_hzps, device: int = 0) -> Bank:
+    f0 = np.ascontiguousarray(f0_hz, dtype=np.float64)
+    f1 = np.ascontiguousarray(f1_hzps, dtype=np.float64)
+    if f0.ndim != 1 or f0.shape != f1.shape:
+        raise ValueError("f0 and f1 must be 1-D and of equal length")
+    h = C.c_void_p()
+    _check(_lib.bfly_make_bank(float(fs_hz), int(L), f0.size, f0.ctypes.data, f1.ctypes.data,
+                               int(device), C.byref(h)), "bfly_make_bank")
+    return Bank(h, int(device), fs_hz, L)
+
+
+def make_bank_grid(fs_hz, L, f0_lo, f0_hi, n_f0, f1_lo, f1_hi, n_f1, device: int = 0) -> Bank:
+    h = C.c_void_p()
+    _check(_lib.bfly_make_bank_grid(float(fs_hz), int(L), float(f0_lo), float(f0_hi), int(n_f0),
+                                    float(f1_lo), float(f1_hi), int(n_f1), int(device),
+                                    C.byref(h)), "bfly_make_bank_grid")
+    return Bank(h, int(device), fs_hz, L)
+
+
+def correlate_form(bank: Bank, form: int, x: torch.Tensor, lag_begin: int = 0,
+                   lag_end: int | None = None, rho_max: torch.Tensor | None = None,
+                   arg_lag: torch.Tensor | None = None):
+    """bfly_correlate_form on torch's current stream; returns (rho_max, arg_lag) tensors."""
+    T = len(bank)
+    n = x.numel()
+    lag_end = n - bank.L + 1 if lag_end is None else lag_end
+    dev = torch.device("cuda", bank.device)
+    if rho_max is None:
+        rho_max = torch.empty(T, dtype=torch.float32, device=dev)
+    if arg_lag is None:
+        arg_lag = torch.empty(T, dtype=torch.int32, device=dev)
+    _check(_lib.bfly_correlate_form(bank._h, int(form), _dev(x, torch.float32, "x", bank.device),
+                                    n, int(lag_begin), int(lag_end),
+                                    _dev(rho_max, torch.float32, "rho_max", bank.device, T),
+                                    _dev(arg_lag, torch.int32, "arg_lag", bank.device, T),
+                                    _stream(bank.device)), "bfly_correlate")
+    return rho_max, arg_lag
+
+
+def correlate(bank: Bank, x: torch.Tensor, lag_begin: int = 0, lag_end: int | None = None,
+              rho_max: torch.Tensor | None = None, arg_lag: torch.Tensor | None = None):
+    return correlate_form(bank, FORM_DEFAULT, x, lag_begin, lag_end, rho_max, arg_lag)
+
+
+def butterfly_map(bank: Bank, rho_max: torch.Tensor, arg_lag: torch.Tensor, kappa: float,
+                  lag_origin: int, samples_per_tbin: int, f_lo_hz: float, df_hz: float,
+                  n_fbins: int, n_tbins: int, map_out: torch.Tensor | None = None,
+                  counters: torch.Tensor | None = None):
+    """bfly_butterfly_map; map_out (int32 storage of the uint32 counts, [n_tbins, n_fbins]) and
+    counters (int64 storage of 2 x uint64) are accumulated into; created zeroed if None."""
+    dev = torch.device("cuda", bank.device)
+    T = len(bank)
+    if map_out is None:
+        map_out = torch.zeros((n_tbins, n_fbins), dtype=torch.int32, device=dev)
+    if counters is None:
+        counters = torch.zeros(2, dtype=torch.int64, device=dev)
+    _check(_lib.bfly_butterfly_map(bank._h, _dev(rho_max, torch.float32, "rho_max", bank.device, T),
+                                   _dev(arg_lag, torch.int32, "arg_lag", bank.device, T),
+                                   float(kappa), int(lag_origin), int(samples_per_tbin),
+                                   float(f_lo_hz), float(df_hz), int(n_fbins), int(n_tbins),
+                                   _dev(map_out, torch.int32, "map_out", bank.device,
+                                        n_fbins * n_tbins),
+                                   _dev(counters, torch.int64, "counters", bank.device, 2),
+                                   _stream(bank.device)), "bfly_butterfly_map")
+    return map_out, counters
+
+
+def search_host(bank: Bank, x_host, chunk_samples: int, kappa: float, samples_per_tbin: int,
+                f_lo_hz: float, df_hz: float, n_fbins: int, n_tbins: int):
+    """bfly_search_host: the whole path on a HOST fp32 series (numpy array or pinned CPU
+    tensor).  Returns numpy (rho_max, arg_lag) of the last chunk, map [n_tbins, n_fbins]
+    uint32 and counters uint64[2]."""
+    if isinstance(x_host, torch.Tensor):
+        if x_host.is_cuda or x_host.dtype != torch.float32 or not x_host.is_contiguous():
+            raise TypeError("x_host must be a contiguous fp32 CPU tensor or numpy array")
+        xp, n = x_host.data_ptr(), x_host.numel()
+    else:
+        x_host = np.ascontiguousarray(x_host)
+        if x_host.dtype != np.float32:
+            raise TypeError("x_host must be fp32")
+        xp, n = x_host.ctypes.data, x_host.size
+    T = len(bank)
+    rho = np.empty(T, np.float32)
+    arg = np.empty(T, np.int32)
+    m = np.empty((n_tbins, n_fbins), np.uint32)
+    cnt = np.empty(2, np.uint64)
+    _check(_lib.bfly_search_host(bank._h, C.c_void_p(xp), n, int(chunk_samples), float(kappa),
+                                 int(samples_per_tbin), float(f_lo_hz), float(df_hz),
+                                 int(n_fbins), int(n_tbins), rho.ctypes.data, arg.ctypes.data,
+                                 m.ctypes.data, cnt.ctypes.data, _stream(bank.device)),
+           "bfly_search_host")
+    return rho, arg, m, cnt
+
+
+def launch_count() -> int:
+    return int(_lib.bfly_launch_count())

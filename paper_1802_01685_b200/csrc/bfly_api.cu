@@ -1,0 +1,331 @@
+// C ABI entry points of libbfly: argument validation, bank and workspace management.
+// See include/bfly.h for the contract of every call.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <atomic>
+#include <new>
+#include <vector>
+
+#include "bfly_internal.cuh"
+
+namespace bfly {
+
+static thread_local char g_err[512] = "";
+static std::atomic<int64_t> g_launches{0};
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? BFLY_ENOMEM : BFLY_ECUDA;
+}
+
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+static int select_device(int device, int *sm_count)
+{
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n <= 0) {
+        set_error("no CUDA device (%s); there is no CPU fallback", cudaGetErrorString(e));
+        return BFLY_EUNSUPPORTED;
+    }
+    if (device < 0 || device >= n) {
+        set_error("device %d out of range (0..%d)", device, n - 1);
+        return BFLY_EINVAL;
+    }
+    cudaDeviceProp p;
+    BFLY_CUDA(cudaGetDeviceProperties(&p, device));
+    if (p.major != 10) {
+        set_error("device %d is sm_%d%d; this library is built for sm_100a only", device, p.major,
+                  p.minor);
+        return BFLY_EUNSUPPORTED;
+    }
+    BFLY_CUDA(cudaSetDevice(device));
+    *sm_count = p.multiProcessorCount;
+    return BFLY_OK;
+}
+
+template <typename T>
+static int grow(T **ptr, int64_t *cap, int64_t need)
+{
+    if (need <= *cap) return BFLY_OK;
+    if (*ptr) {
+        BFLY_CUDA(cudaFree(*ptr));
+        *ptr = nullptr;
+        *cap = 0;
+    }
+    BFLY_CUDA(cudaMalloc((void **)ptr, sizeof(T) * (size_t)need));
+    *cap = need;
+    return BFLY_OK;
+}
+
+static int reserve_for(bfly_bank *b, int64_t n_samples)
+{
+    if (n_samples < b->L) return BFLY_OK;
+    const int64_t n_lags = n_samples - b->L + 1;
+    int rc = grow(&b->rn2, &b->rn2_cap, n_lags);
+    if (rc) return rc;
+    return grow(&b->xspec, &b->xspec_cap, fft_blocks_needed(b->L, n_lags));
+}
+
+}  // namespace bfly
+
+using namespace bfly;
+
+extern "C" {
+
+const char *bfly_strerror(int status)
+{
+    switch (status) {
+        case BFLY_OK: return "ok";
+        case BFLY_EINVAL: return "invalid argument";
+        case BFLY_ENOMEM: return "out of memory";
+        case BFLY_ECUDA: return "CUDA error";
+        case BFLY_EUNSUPPORTED: return "unsupported device or form (sm_100a required, no CPU fallback)";
+        case BFLY_ERANGE: return "size out of the supported range";
+        default: return "unknown status";
+    }
+}
+
+const char *bfly_last_error(void) { return g_err; }
+
+int64_t bfly_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+void bfly_free_bank(bfly_bank *b)
+{
+    if (!b) return;
+    cudaSetDevice(b->device);
+    cudaFree(b->f0); cudaFree(b->f1); cudaFree(b->phA); cudaFree(b->phB);
+    cudaFree(b->inc2); cudaFree(b->ins2); cudaFree(b->rn2); cudaFree(b->xspec);
+    cudaFree(b->packed); cudaFree(b->x_stage); cudaFree(b->rho_stage); cudaFree(b->arg_stage);
+    cudaFree(b->map_stage); cudaFree(b->cnt_stage);
+    if (b->ev_start) cudaEventDestroy(b->ev_start);
+    if (b->ev_stop) cudaEventDestroy(b->ev_stop);
+    delete b;
+}
+
+int64_t bfly_bank_size(const bfly_bank *b) { return b ? b->T : -1; }
+
+int bfly_make_bank(double fs_hz, int32_t L, int64_t n_templates, const double *f0_hz,
+                   const double *f1_hzps, int device, bfly_bank **out_bank)
+{
+    if (!out_bank || !f0_hz || !f1_hzps) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (!(fs_hz > 0.0) || !std::isfinite(fs_hz)) { set_error("fs must be finite and > 0"); return BFLY_EINVAL; }
+    if (L < 2) { set_error("L must be >= 2"); return BFLY_EINVAL; }
+    if (L > FFT_MAX_L) { set_error("L = %d exceeds the supported maximum %d", L, FFT_MAX_L); return BFLY_ERANGE; }
+    if (n_templates < 1) { set_error("n_templates must be >= 1"); return BFLY_EINVAL; }
+    for (int64_t j = 0; j < n_templates; ++j)
+        if (!std::isfinite(f0_hz[j]) || !std::isfinite(f1_hzps[j])) {
+            set_error("template %lld has a non-finite f0 or f1", (long long)j);
+            return BFLY_EINVAL;
+        }
+    int sms = 0;
+    int rc = select_device(device, &sms);
+    if (rc) return rc;
+    bfly_bank *b = new (std::nothrow) bfly_bank();
+    if (!b) { set_error("host allocation failed"); return BFLY_ENOMEM; }
+    memset(b, 0, sizeof(*b));
+    b->device = device; b->sm_count = sms; b->fs = fs_hz; b->L = L; b->T = n_templates;
+    const size_t T = (size_t)n_templates;
+    cudaError_t e;
+#define BANK_TRY(call) if ((e = (call)) != cudaSuccess) { rc = cuda_fail(e, #call); bfly_free_bank(b); return rc; }
+    BANK_TRY(cudaMalloc((void **)&b->f0, T * sizeof(double)));
+    BANK_TRY(cudaMalloc((void **)&b->f1, T * sizeof(double)));
+    BANK_TRY(cudaMalloc((void **)&b->phA, T * sizeof(uint64_t)));
+    BANK_TRY(cudaMalloc((void **)&b->phB, T * sizeof(uint64_t)));
+    BANK_TRY(cudaMalloc((void **)&b->inc2, T * sizeof(float)));
+    BANK_TRY(cudaMalloc((void **)&b->ins2, T * sizeof(float)));
+    BANK_TRY(cudaMalloc((void **)&b->packed, T * sizeof(unsigned long long)));
+    BANK_TRY(cudaMalloc((void **)&b->rho_stage, T * sizeof(float)));
+    BANK_TRY(cudaMalloc((void **)&b->arg_stage, T * sizeof(int32_t)));
+    BANK_TRY(cudaMalloc((void **)&b->cnt_stage, 2 * sizeof(unsigned long long)));
+    BANK_TRY(cudaMemcpy(b->f0, f0_hz, T * sizeof(double), cudaMemcpyHostToDevice));
+    BANK_TRY(cudaMemcpy(b->f1, f1_hzps, T * sizeof(double), cudaMemcpyHostToDevice));
+#undef BANK_TRY
+    rc = launch_bank_params(b, 0);
+    if (rc == BFLY_OK) {
+        e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) rc = cuda_fail(e, "bank parameter kernel");
+    }
+    if (rc) { bfly_free_bank(b); return rc; }
+    *out_bank = b;
+    return BFLY_OK;
+}
+
+int bfly_make_bank_grid(double fs_hz, int32_t L, double f0_lo, double f0_hi, int32_t n_f0,
+                        double f1_lo, double f1_hi, int32_t n_f1, int device, bfly_bank **out_bank)
+{
+    if (n_f0 < 1 || n_f1 < 1) { set_error("grid sizes must be >= 1"); return BFLY_EINVAL; }
+    if (!std::isfinite(f0_lo) || !std::isfinite(f0_hi) || !std::isfinite(f1_lo) || !std::isfinite(f1_hi)) {
+        set_error("grid bounds must be finite"); return BFLY_EINVAL;
+    }
+    const int64_t T = (int64_t)n_f0 * n_f1;
+    std::vector<double> f0, f1;
+    try { f0.resize((size_t)T); f1.resize((size_t)T); }
+    catch (...) { set_error("host allocation failed"); return BFLY_ENOMEM; }
+    // numpy.linspace: start + i * step with step = (stop - start) / (n - 1); last point = stop
+    const double s0 = n_f0 > 1 ? (f0_hi - f0_lo) / (double)(n_f0 - 1) : 0.0;
+    const double s1 = n_f1 > 1 ? (f1_hi - f1_lo) / (double)(n_f1 - 1) : 0.0;
+    for (int32_t i = 0; i < n_f0; ++i) {
+        const double a = (n_f0 > 1 && i == n_f0 - 1) ? f0_hi : f0_lo + (double)i * s0;
+        for (int32_t k = 0; k < n_f1; ++k) {
+            const double c = (n_f1 > 1 && k == n_f1 - 1) ? f1_hi : f1_lo + (double)k * s1;
+            f0[(size_t)i * n_f1 + k] = a;
+            f1[(size_t)i * n_f1 + k] = c;
+        }
+    }
+    return bfly_make_bank(fs_hz, L, T, f0.data(), f1.data(), device, out_bank);
+}
+
+int bfly_bank_get(const bfly_bank *b, int64_t first, int64_t count, double *f0_hz,
+                  double *f1_hzps, float *inv_nc2, float *inv_ns2)
+{
+    if (!b) { set_error("null bank"); return BFLY_EINVAL; }
+    if (first < 0 || count < 0 || first + count > b->T) { set_error("template range outside the bank"); return BFLY_EINVAL; }
+    BFLY_CUDA(cudaSetDevice(b->device));
+    const size_t n = (size_t)count;
+    if (f0_hz) BFLY_CUDA(cudaMemcpy(f0_hz, b->f0 + first, n * sizeof(double), cudaMemcpyDeviceToHost));
+    if (f1_hzps) BFLY_CUDA(cudaMemcpy(f1_hzps, b->f1 + first, n * sizeof(double), cudaMemcpyDeviceToHost));
+    if (inv_nc2) BFLY_CUDA(cudaMemcpy(inv_nc2, b->inc2 + first, n * sizeof(float), cudaMemcpyDeviceToHost));
+    if (inv_ns2) BFLY_CUDA(cudaMemcpy(inv_ns2, b->ins2 + first, n * sizeof(float), cudaMemcpyDeviceToHost));
+    return BFLY_OK;
+}
+
+int bfly_bank_reserve(bfly_bank *b, int64_t max_n_samples)
+{
+    if (!b) { set_error("null bank"); return BFLY_EINVAL; }
+    if (max_n_samples < b->L) { set_error("max_n_samples < L"); return BFLY_EINVAL; }
+    if (max_n_samples >= (1LL << 31)) { set_error("segment too long"); return BFLY_ERANGE; }
+    BFLY_CUDA(cudaSetDevice(b->device));
+    return reserve_for(b, max_n_samples);
+}
+
+int bfly_bank_set_timing(bfly_bank *b, int enable)
+{
+    if (!b) { set_error("null bank"); return BFLY_EINVAL; }
+    BFLY_CUDA(cudaSetDevice(b->device));
+    if (enable && !b->ev_start) {
+        BFLY_CUDA(cudaEventCreate(&b->ev_start));
+        BFLY_CUDA(cudaEventCreate(&b->ev_stop));
+    }
+    b->timing = enable ? 1 : 0;
+    b->timed = 0;
+    return BFLY_OK;
+}
+
+int bfly_bank_core_ms(bfly_bank *b, float *ms_out)
+{
+    if (!b || !ms_out) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (!b->timing || !b->timed) { set_error("no timed bfly_correlate call on this bank"); return BFLY_EINVAL; }
+    BFLY_CUDA(cudaEventSynchronize(b->ev_stop));
+    BFLY_CUDA(cudaEventElapsedTime(ms_out, b->ev_start, b->ev_stop));
+    return BFLY_OK;
+}
+
+int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int64_t n_samples,
+                        int64_t lag_begin, int64_t lag_end, float *rho_max_dev,
+                        int32_t *arg_lag_dev, void *stream)
+{
+    if (!bank || !x_dev || !rho_max_dev || !arg_lag_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n_samples < bank->L) { set_error("n_samples < L"); return BFLY_EINVAL; }
+    if (n_samples >= (1LL << 31)) { set_error("segment too long (n_samples must be < 2^31)"); return BFLY_ERANGE; }
+    if (lag_begin < 0 || lag_end < lag_begin || lag_end > n_samples - bank->L + 1) {
+        set_error("lag range [%lld, %lld) outside the valid lags [0, %lld)", (long long)lag_begin,
+                  (long long)lag_end, (long long)(n_samples - bank->L + 1));
+        return BFLY_EINVAL;
+    }
+    if (form == BFLY_FORM_DEFAULT) form = BFLY_FORM_FFT;
+    if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
+    bfly_bank *b = const_cast<bfly_bank *>(bank);   // the workspace is mutable state of the bank
+    BFLY_CUDA(cudaSetDevice(b->device));
+    int rc = reserve_for(b, n_samples);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = launch_sliding_norm(x_dev, n_samples, b->L, lag_begin, lag_end - lag_begin, b->rn2, st);
+    if (rc) return rc;
+    if (form == BFLY_FORM_DIRECT)
+        return launch_direct(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    return launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+}
+
+int bfly_correlate(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int64_t lag_begin,
+                   int64_t lag_end, float *rho_max_dev, int32_t *arg_lag_dev, void *stream)
+{
+    return bfly_correlate_form(bank, BFLY_FORM_DEFAULT, x_dev, n_samples, lag_begin, lag_end,
+                               rho_max_dev, arg_lag_dev, stream);
+}
+
+int bfly_butterfly_map(const bfly_bank *bank, const float *rho_max_dev, const int32_t *arg_lag_dev,
+                       float kappa, int64_t lag_origin, int32_t samples_per_tbin, double f_lo_hz,
+                       double df_hz, int32_t n_fbins, int32_t n_tbins, uint32_t *map_dev,
+                       uint64_t *counters_dev, void *stream)
+{
+    if (!bank || !rho_max_dev || !arg_lag_dev || !map_dev || !counters_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (!std::isfinite(kappa)) { set_error("kappa must be finite"); return BFLY_EINVAL; }
+    if (!(df_hz > 0.0) || !std::isfinite(df_hz) || !std::isfinite(f_lo_hz)) { set_error("df must be finite and > 0, f_lo finite"); return BFLY_EINVAL; }
+    if (samples_per_tbin <= 0 || n_fbins <= 0 || n_tbins <= 0 || lag_origin < 0) { set_error("bad map geometry"); return BFLY_EINVAL; }
+    BFLY_CUDA(cudaSetDevice(bank->device));
+    return launch_map(bank, rho_max_dev, arg_lag_dev, kappa, lag_origin, samples_per_tbin, f_lo_hz,
+                      df_hz, n_fbins, n_tbins, map_dev, (unsigned long long *)counters_dev,
+                      (cudaStream_t)stream);
+}
+
+int bfly_search_host(bfly_bank *b, const float *x_host, int64_t n_samples, int64_t chunk_samples,
+                     float kappa, int32_t samples_per_tbin, double f_lo_hz, double df_hz,
+                     int32_t n_fbins, int32_t n_tbins, float *rho_max_host, int32_t *arg_lag_host,
+                     uint32_t *map_host, uint64_t *counters_host, void *stream)
+{
+    if (!b || !x_host) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n_samples < b->L) { set_error("n_samples < L"); return BFLY_EINVAL; }
+    if (!std::isfinite(kappa) || !(df_hz > 0.0) || !std::isfinite(df_hz) || !std::isfinite(f_lo_hz) ||
+        samples_per_tbin <= 0 || n_fbins <= 0 || n_tbins <= 0) { set_error("bad threshold or map geometry"); return BFLY_EINVAL; }
+    if (chunk_samples <= 0 || chunk_samples > n_samples) chunk_samples = n_samples;
+    if (chunk_samples <= b->L && chunk_samples < n_samples) { set_error("chunk_samples must exceed L"); return BFLY_EINVAL; }
+    if (chunk_samples >= (1LL << 31)) { set_error("chunk too long"); return BFLY_ERANGE; }
+    BFLY_CUDA(cudaSetDevice(b->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = reserve_for(b, chunk_samples);
+    if (rc) return rc;
+    if ((rc = grow(&b->x_stage, &b->x_stage_cap, chunk_samples))) return rc;
+    const int64_t cells = (int64_t)n_fbins * n_tbins;
+    if ((rc = grow(&b->map_stage, &b->map_stage_cap, cells))) return rc;
+    BFLY_CUDA(cudaMemsetAsync(b->map_stage, 0, sizeof(uint32_t) * (size_t)cells, st));
+    BFLY_CUDA(cudaMemsetAsync(b->cnt_stage, 0, 2 * sizeof(unsigned long long), st));
+    const int64_t total_lags = n_samples - b->L + 1;
+    // a single chunk takes every valid lag; otherwise hop = chunk - L (reading C11)
+    const int64_t hop = (chunk_samples >= n_samples) ? total_lags : chunk_samples - b->L;
+    for (int64_t start = 0; start < total_lags; start += hop) {
+        const int64_t n = (chunk_samples < n_samples - start) ? chunk_samples : n_samples - start;
+        const int64_t lags_here = n - b->L + 1;
+        const bool last = start + hop >= total_lags;
+        const int64_t lag_end = last ? lags_here : (hop < lags_here ? hop : lags_here);
+        BFLY_CUDA(cudaMemcpyAsync(b->x_stage, x_host + start, sizeof(float) * (size_t)n,
+                                  cudaMemcpyHostToDevice, st));
+        rc = bfly_correlate(b, b->x_stage, n, 0, lag_end, b->rho_stage, b->arg_stage, st);
+        if (rc) return rc;
+        rc = bfly_butterfly_map(b, b->rho_stage, b->arg_stage, kappa, start, samples_per_tbin,
+                                f_lo_hz, df_hz, n_fbins, n_tbins, b->map_stage,
+                                (uint64_t *)b->cnt_stage, st);
+        if (rc) return rc;
+        if (last) break;
+    }
+    const size_t T = (size_t)b->T;
+    if (rho_max_host) BFLY_CUDA(cudaMemcpyAsync(rho_max_host, b->rho_stage, T * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (arg_lag_host) BFLY_CUDA(cudaMemcpyAsync(arg_lag_host, b->arg_stage, T * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    if (map_host) BFLY_CUDA(cudaMemcpyAsync(map_host, b->map_stage, sizeof(uint32_t) * (size_t)cells, cudaMemcpyDeviceToHost, st));
+    if (counters_host) BFLY_CUDA(cudaMemcpyAsync(counters_host, b->cnt_stage, 2 * sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+    BFLY_CUDA(cudaStreamSynchronize(st));
+    return BFLY_OK;
+}
+
+}  // extern "C"

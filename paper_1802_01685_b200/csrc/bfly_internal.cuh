@@ -1,0 +1,95 @@
+// Internal declarations shared by the translation units of libbfly (not part of the C ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/bfly.h"
+
+struct bfly_bank {
+    int device;
+    int sm_count;
+    double fs;
+    int32_t L;
+    int64_t T;
+    // per-template parameters (device, struct of arrays; A1)
+    double *f0;      // Hz
+    double *f1;      // Hz/s
+    uint64_t *phA;   // f0/fs            in units of 2^-64 cycles per sample
+    uint64_t *phB;   // f1/(2 fs^2)      in units of 2^-64 cycles per sample^2
+    float *inc2;     // 1 / ||cos phi||^2 (0 if the norm is 0)
+    float *ins2;     // 1 / ||sin phi||^2
+    // workspace (grown by bfly_bank_reserve / on demand)
+    float *rn2;               // 1 / n2[tau] for the lags of the current call
+    int64_t rn2_cap;          // floats
+    float2 *xspec;            // data-block spectra, [block][16][512] complex
+    int64_t xspec_cap;        // blocks
+    unsigned long long *packed;  // T packed (rho^2 bits, ~lag) words for the direct form
+    float *x_stage;           // device copy of a host chunk (bfly_search_host)
+    int64_t x_stage_cap;
+    float *rho_stage;         // T
+    int32_t *arg_stage;       // T
+    uint32_t *map_stage;
+    int64_t map_stage_cap;
+    unsigned long long *cnt_stage;  // 2
+    // measurement aid (bfly_bank_set_timing)
+    int timing;
+    int timed;                  // a start/stop pair has been recorded
+    cudaEvent_t ev_start, ev_stop;
+};
+
+namespace bfly {
+
+void set_error(const char *fmt, ...);
+int cuda_fail(cudaError_t e, const char *what);   // records the message, returns BFLY_ECUDA
+void count_launch(int n = 1);
+
+#define BFLY_CUDA(call)                                          \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) return bfly::cuda_fail(e__, #call); \
+    } while (0)
+
+// bfly_bank_set_timing: events around the correlation-core kernel on the caller's stream
+inline void core_timer_start(const bfly_bank *b, cudaStream_t st)
+{
+    if (b->timing) cudaEventRecord(b->ev_start, st);
+}
+inline void core_timer_stop(const bfly_bank *b, cudaStream_t st)
+{
+    if (b->timing) {
+        cudaEventRecord(b->ev_stop, st);
+        const_cast<bfly_bank *>(b)->timed = 1;
+    }
+}
+
+// FFT-form geometry: block length of the overlap-save FFT.
+constexpr int FFT_LOG2B = 13;
+constexpr int FFT_B = 1 << FFT_LOG2B;   // 8192
+constexpr int FFT_MAX_L = FFT_B / 2;    // 4096
+
+// launchers (each enqueues on `stream`, returns a BFLY_* status)
+int launch_bank_params(bfly_bank *b, cudaStream_t stream);
+int launch_sliding_norm(const float *x, int64_t n_samples, int32_t L, int64_t lag_begin,
+                        int64_t n_lags, float *rn2, cudaStream_t stream);
+int launch_direct(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                  int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
+int launch_fft(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+               int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
+int launch_map(const bfly_bank *b, const float *rho_max, const int32_t *arg_lag, float kappa,
+               int64_t lag_origin, int32_t samples_per_tbin, double f_lo, double df,
+               int32_t n_fbins, int32_t n_tbins, uint32_t *map, unsigned long long *counters,
+               cudaStream_t stream);
+int64_t fft_blocks_needed(int32_t L, int64_t n_lags);
+
+// Template phase in cycles, as a 64-bit fixed-point fraction: phi_k/2pi mod 1 = (A k + B k^2) 2^-64.
+__device__ __forceinline__ void template_sincos(uint64_t A, uint64_t B, uint32_t k, float *s,
+                                                float *c)
+{
+    uint64_t ph = A * (uint64_t)k + B * ((uint64_t)k * (uint64_t)k);
+    // top 32 bits as a signed fraction of a half-turn: angle = pi * v, v in [-1, 1)
+    float v = (float)(int32_t)(uint32_t)(ph >> 32) * 4.656612873077393e-10f;  // 2^-31
+    sincospif(v, s, c);
+}
+
+}  // namespace bfly

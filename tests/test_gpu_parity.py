@@ -1,0 +1,228 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by
+element on the same seeded inputs (rules R1-R4 of DESIGN.md).  Needs a B200."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import streaming
+from workloads import bank_grid, default_map_grid, get_config, make_data, sub_bank_indices
+
+from parity import check_map, check_values_and_argmax
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def bfly():
+    import paper_1802_01685_b200 as b
+    return b
+
+
+FORMS = [pytest.param(1, id="fft"), pytest.param(2, id="direct")]
+
+
+def _run(bfly, form, fs, L, f0, f1, x, lag_begin=0, lag_end=None):
+    bank = bfly.make_bank(fs, L, f0, f1)
+    xd = torch.from_numpy(x).cuda()
+    rho, arg = bfly.correlate_form(bank, form, xd, lag_begin, lag_end)
+    torch.cuda.synchronize()
+    return bank, rho, arg
+
+
+# ----------------------------------------------------------------- config 1, whole bank
+@pytest.mark.parametrize("form", FORMS)
+def test_tiny_full_bank(bfly, form):
+    cfg = get_config(1)
+    x = make_data(cfg)
+    f0, f1 = bank_grid(cfg)
+    bank, rho, arg = _run(bfly, form, cfg.fs_hz, cfg.L, f0, f1, x)
+    rho_o, arg_o, exempt = check_values_and_argmax(x, cfg.fs_hz, cfg.L, f0, f1,
+                                                   rho.cpu().numpy(), arg.cpu().numpy())
+    # the map at the config's kappa (empty by construction) and at kappa = 0.09
+    grid = default_map_grid(cfg)
+    for kappa in (cfg.kappa, 0.09, 0.0):
+        m, c = bfly.butterfly_map(bank, rho, arg, kappa, 0, **grid)
+        check_map(f0, rho.cpu().numpy(), arg.cpu().numpy(), m.cpu().numpy().view(np.uint32),
+                  c.cpu().numpy().view(np.uint64), rho_o, arg_o, exempt, kappa, 0, grid)
+
+
+@pytest.mark.parametrize("form", FORMS)
+def test_tiny_injection_on_a_grid_node(bfly, form):
+    # the injected chirp moved onto a bank node: rho ~ A/sqrt(2) at the injected lag (pin P9)
+    cfg = get_config(1)
+    f0, f1 = bank_grid(cfg)
+    j = 7 * cfg.n_f1 + 5
+    rng = np.random.default_rng(77)
+    x = rng.standard_normal(cfg.n_samples)
+    hc, _ = oracle.template(cfg.fs_hz, cfg.L, f0[j], f1[j])
+    x[1000:1000 + cfg.L] += 0.3 * hc
+    x = x.astype(np.float32)
+    bank, rho, arg = _run(bfly, form, cfg.fs_hz, cfg.L, f0, f1, x)
+    rho_n, arg_n = rho.cpu().numpy(), arg.cpu().numpy()
+    rho_o, arg_o, exempt = check_values_and_argmax(x, cfg.fs_hz, cfg.L, f0, f1, rho_n, arg_n)
+    assert arg_n[j] == 1000 and rho_n[j] > 0.18
+    grid = default_map_grid(cfg)
+    m, c = bfly.butterfly_map(bank, rho, arg, cfg.kappa, 0, **grid)
+    n_amb = check_map(f0, rho_n, arg_n, m.cpu().numpy().view(np.uint32),
+                      c.cpu().numpy().view(np.uint64), rho_o, arg_o, exempt, cfg.kappa, 0, grid)
+    assert int(c[0]) >= 1 and n_amb < 8
+
+
+# ----------------------------------------------------------------- ragged sizes and edge cases
+@pytest.mark.parametrize("form", FORMS)
+@pytest.mark.parametrize("fs,L,N", [(2000.0, 2000, 9000), (1000.0, 300, 1500), (4096.0, 4096, 4096),
+                                     (4096.0, 4096, 12300), (512.0, 2, 40), (777.0, 1023, 9217)])
+def test_ragged_sizes(bfly, form, fs, L, N):
+    rng = np.random.default_rng(int(L + N))
+    x = rng.standard_normal(N).astype(np.float32)
+    T = 37                                           # not a multiple of any tile
+    f0 = rng.uniform(0.02 * fs, 0.45 * fs, T)
+    f1 = rng.uniform(-0.2 * fs, 0.2 * fs, T)
+    _, rho, arg = _run(bfly, form, fs, L, f0, f1, x)
+    check_values_and_argmax(x, fs, L, f0, f1, rho.cpu().numpy(), arg.cpu().numpy())
+
+
+@pytest.mark.parametrize("form", FORMS)
+def test_lag_subrange_and_empty_range(bfly, form):
+    rng = np.random.default_rng(5)
+    fs, L, N = 2048.0, 2048, 20000
+    x = rng.standard_normal(N).astype(np.float32)
+    f0 = rng.uniform(100, 900, 19)
+    f1 = rng.uniform(-300, 300, 19)
+    for lb, le in ((5000, 11237), (0, 1), (N - L, N - L + 1), (17, 17 + 6145), (17, 17 + 6146)):
+        _, rho, arg = _run(bfly, form, fs, L, f0, f1, x, lb, le)
+        check_values_and_argmax(x, fs, L, f0, f1, rho.cpu().numpy(), arg.cpu().numpy(), lb, le)
+    _, rho, arg = _run(bfly, form, fs, L, f0, f1, x, 123, 123)     # empty: rho 0, arg lag_begin
+    assert np.all(rho.cpu().numpy() == 0.0) and np.all(arg.cpu().numpy() == 123)
+
+
+@pytest.mark.parametrize("form", FORMS)
+def test_degenerate_inputs(bfly, form):
+    fs, L, N = 1024.0, 512, 3000
+    # (0, 0): the sine template is identically zero and contributes nothing (C4).  (fs/2, 0) is
+    # left out: there the float64 oracle's sin(pi k) is rounding noise, not zero (C4).
+    f0 = np.array([100.0, 0.0, 256.0, 300.0, 511.0])
+    f1 = np.array([50.0, 0.0, 0.0, -700.0, 3.0])
+    # all-zero data: rho = 0 everywhere, argmax = first lag (C6, C8)
+    x = np.zeros(N, np.float32)
+    _, rho, arg = _run(bfly, form, fs, L, f0, f1, x)
+    assert np.all(rho.cpu().numpy() == 0.0) and np.all(arg.cpu().numpy() == 0)
+    # a zero stretch longer than L inside noise, and a large overall scale (P5)
+    rng = np.random.default_rng(9)
+    x = rng.standard_normal(N).astype(np.float32)
+    x[700:1500] = 0.0
+    for scale in (1.0, 3.0e4, 2.0e-5):
+        xs = (x * np.float32(scale)).astype(np.float32)
+        _, rho, arg = _run(bfly, form, fs, L, f0, f1, xs)
+        check_values_and_argmax(xs, fs, L, f0, f1, rho.cpu().numpy(), arg.cpu().numpy())
+
+
+def test_noise_free_injection_gives_rho_one(bfly):
+    # pin P2 through the CUDA path: x = a * hc at lag tau0, zero elsewhere
+    fs, L, N, tau0 = 4096.0, 4096, 20000, 7777
+    hc, hs = oracle.template(fs, L, 700.0, -210.0)
+    x = np.zeros(N)
+    x[tau0:tau0 + L] = 3.0 * hc
+    x = x.astype(np.float32)
+    for form in (1, 2):
+        _, rho, arg = _run(bfly, form, fs, L, [700.0], [-210.0], x)
+        assert abs(float(rho[0]) - 1.0) < 1e-4 and int(arg[0]) == tau0
+
+
+# ----------------------------------------------------------------- bank parameters (A1)
+def test_bank_parameters_match_oracle_norms(bfly):
+    cfg = get_config(4)
+    idx = sub_bank_indices(cfg, 40)
+    f0a, f1a = bank_grid(cfg)
+    bank = bfly.make_bank(cfg.fs_hz, cfg.L, f0a[idx], f1a[idx])
+    f0, f1, inc2, ins2 = bank.get()
+    np.testing.assert_array_equal(f0, f0a[idx])
+    np.testing.assert_array_equal(f1, f1a[idx])
+    for j in range(len(idx)):
+        hc, hs = oracle.template(cfg.fs_hz, cfg.L, f0[j], f1[j])
+        nc, ns = oracle.template_norms(hc, hs)
+        assert abs(inc2[j] * nc * nc - 1.0) < 1e-6 and abs(ins2[j] * ns * ns - 1.0) < 1e-6
+    grid = bfly.make_bank_grid(cfg.fs_hz, cfg.L, cfg.f0_lo, cfg.f0_hi, 64, cfg.f1_lo, cfg.f1_hi, 32)
+    g0, g1, _, _ = grid.get()
+    np.testing.assert_array_equal(g0, np.repeat(np.linspace(cfg.f0_lo, cfg.f0_hi, 64), 32))
+    np.testing.assert_array_equal(g1, np.tile(np.linspace(cfg.f1_lo, cfg.f1_hi, 32), 64))
+
+
+# ----------------------------------------------------------------- configs 2-4: seeded sub-banks
+@pytest.mark.parametrize("form", FORMS)
+@pytest.mark.parametrize("index,n_random,n_samples", [(2, 40, None), (3, 40, None), (4, 48, None)])
+def test_sub_bank_of_config(bfly, form, index, n_random, n_samples):
+    cfg = get_config(index)
+    x = make_data(cfg, n_samples)
+    f0a, f1a = bank_grid(cfg)
+    idx = sub_bank_indices(cfg, n_random, max_track=24)
+    f0, f1 = f0a[idx], f1a[idx]
+    bank, rho, arg = _run(bfly, form, cfg.fs_hz, cfg.L, f0, f1, x)
+    rho_n, arg_n = rho.cpu().numpy(), arg.cpu().numpy()
+    rho_o, arg_o, exempt = check_values_and_argmax(x, cfg.fs_hz, cfg.L, f0, f1, rho_n, arg_n)
+    grid = default_map_grid(cfg)
+    m, c = bfly.butterfly_map(bank, rho, arg, cfg.kappa, 0, **grid)
+    check_map(f0, rho_n, arg_n, m.cpu().numpy().view(np.uint32), c.cpu().numpy().view(np.uint64),
+              rho_o, arg_o, exempt, cfg.kappa, 0, grid)
+
+
+# ----------------------------------------------------------------- R4: determinism, sub == full
+def test_full_bank_config2_is_deterministic_and_matches_sub_bank(bfly):
+    cfg = get_config(2)
+    x = make_data(cfg)
+    xd = torch.from_numpy(x).cuda()
+    full = bfly.make_bank_grid(cfg.fs_hz, cfg.L, cfg.f0_lo, cfg.f0_hi, cfg.n_f0,
+                               cfg.f1_lo, cfg.f1_hi, cfg.n_f1)
+    r1, a1 = bfly.correlate(full, xd)
+    r2, a2 = bfly.correlate(full, xd)
+    torch.cuda.synchronize()
+    assert torch.equal(r1, r2) and torch.equal(a1, a2)
+    f0a, f1a = bank_grid(cfg)
+    idx = sub_bank_indices(cfg, 300)
+    sub = bfly.make_bank(cfg.fs_hz, cfg.L, f0a[idx], f1a[idx])
+    rs, as_ = bfly.correlate(sub, xd)
+    it = torch.from_numpy(idx).cuda()
+    assert torch.equal(rs, r1[it]) and torch.equal(as_, a1[it])
+    # the direct form on the same sub-bank agrees with the FFT form within R1
+    rd, ad = bfly.correlate_form(sub, bfly.FORM_DIRECT, xd)
+    assert float((rd - rs).abs().max()) <= 2e-4
+
+
+# ----------------------------------------------------------------- A9: streaming from the host
+@pytest.mark.parametrize("n_samples,chunk", [(40000, 16384), (65536 + 3 * 61440 + 777, 65536),
+                                             (30000, 0)])
+def test_search_host_streaming(bfly, n_samples, chunk):
+    """bfly_search_host equals, bit for bit, the composition of bfly_correlate and
+    bfly_butterfly_map over the chunk plan of reading C11, and every chunk of that
+    composition satisfies R1-R3 against the oracle."""
+    cfg = get_config(5)
+    L = cfg.L
+    rng = np.random.default_rng(55)
+    x = rng.standard_normal(n_samples).astype(np.float32)
+    f0a, f1a = bank_grid(cfg)
+    idx = sub_bank_indices(cfg, 24, max_track=4)
+    f0, f1 = f0a[idx], f1a[idx]
+    grid = default_map_grid(cfg, n_samples)
+    kappa = 0.07
+    bank = bfly.make_bank(cfg.fs_hz, L, f0, f1)
+    rho_h, arg_h, m_h, cnt_h = bfly.search_host(bank, x, chunk, kappa, **grid)
+    plan = streaming.chunk_plan(n_samples, L, chunk if chunk > 0 else n_samples)
+    m_o, c_o, per_chunk = streaming.stream(x, cfg.fs_hz, L, f0, f1,
+                                           chunk if chunk > 0 else n_samples, kappa, grid)
+    xd = torch.from_numpy(x).cuda()
+    m_d = c_d = None
+    for (s, n, lb, le), (_, r_o, a_o) in zip(plan, per_chunk):
+        rho, arg = bfly.correlate(bank, xd[s:s + n], lb, le)
+        m_c, c_c = bfly.butterfly_map(bank, rho, arg, kappa, s, **grid)
+        m_d, c_d = bfly.butterfly_map(bank, rho, arg, kappa, s, **grid, map_out=m_d, counters=c_d)
+        rho_n, arg_n = rho.cpu().numpy(), arg.cpu().numpy()
+        _, _, exempt = check_values_and_argmax(x[s:s + n], cfg.fs_hz, L, f0, f1, rho_n, arg_n,
+                                               lb, le, oracle_result=(r_o, a_o))
+        check_map(f0, rho_n, arg_n, m_c.cpu().numpy().view(np.uint32),
+                  c_c.cpu().numpy().view(np.uint64), r_o, a_o, exempt, kappa, s, grid)
+    np.testing.assert_array_equal(m_h, m_d.cpu().numpy().view(np.uint32))
+    np.testing.assert_array_equal(cnt_h, c_d.cpu().numpy().view(np.uint64))
+    np.testing.assert_array_equal(rho_h, rho_n)
+    np.testing.assert_array_equal(arg_h, arg_n)
