@@ -62,7 +62,8 @@ def test_tiny_injection_on_a_grid_node(bfly, form):
     bank, rho, arg = _run(bfly, form, cfg.fs_hz, cfg.L, f0, f1, x)
     rho_n, arg_n = rho.cpu().numpy(), arg.cpu().numpy()
     rho_o, arg_o, exempt = check_values_and_argmax(x, cfg.fs_hz, cfg.L, f0, f1, rho_n, arg_n)
-    assert arg_n[j] == 1000 and rho_n[j] > 0.18
+    # noise moves the maximum by at most one lag from the injected start (oracle: 1001)
+    assert arg_n[j] == arg_o[j] and abs(int(arg_n[j]) - 1000) <= 1 and rho_n[j] > 0.18
     grid = default_map_grid(cfg)
     m, c = bfly.butterfly_map(bank, rho, arg, cfg.kappa, 0, **grid)
     n_amb = check_map(f0, rho_n, arg_n, m.cpu().numpy().view(np.uint32),
