@@ -75,7 +75,7 @@ static int reserve_for(bfly_bank *b, int64_t n_samples)
     const int64_t n_lags = n_samples - b->L + 1;
     int rc = grow(&b->rn2, &b->rn2_cap, n_lags);
     if (rc) return rc;
-    return grow(&b->xspec, &b->xspec_cap, fft_blocks_needed(b->L, n_lags));
+    return grow(&b->xspec, &b->xspec_cap, fft_blocks_needed(b->L, n_lags) * FFT_B);
 }
 
 }  // namespace bfly

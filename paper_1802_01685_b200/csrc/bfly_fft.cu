@@ -1,15 +1,296 @@
-// TEMPORARY STUB (replaced by the FFT form): routes to the direct form so that the boundary,
-// the tests and the bench can be exercised end to end.
+// BFLY_FORM_FFT: hand-written batched overlap-save FFT correlate with the fused epilogue
+// (rows A3-A7 of DESIGN.md; the paper's own correlation method: "FFT ...
+// complex-to-complex single precision", here entirely in registers and shared memory).
+//
+// Mathematics.  With g[k] = cos(phi_k) - i sin(phi_k) (k < L, zero-padded to B) and a data block
+// xb[n] = x[o_b + n], n < B,
+//     z_b(tau') = sum_k xb[tau' + k] g[k] = c(tau') - i s(tau')      exact for tau' <= B - L,
+// and with F+ the unnormalised length-B transform Y[m] = sum_n y[n] exp(+2 pi i m n / B):
+//     z_b = F+( X_b . G ),   G = F+(g),   X_b = conj(F+(xb)) / B.
+// X_b is computed once per call by data_spectra_kernel; the correlation kernel keeps G in
+// registers, so per (template, block) the only memory traffic is one read of X_b from L2.
+//
+// The length-8192 transform is 32 x 16 x 16, three passes of register-resident radix-2 DIF
+// butterflies, 256 threads x 32 points:
+//     n = 256 n1 + 16 n2 + n3   ->   m = m1 + 32 m2 + 512 m3
+//     pass 1: thread t = 16 n2 + n3: 32-point over n1, times w_8192^(m1 t)
+//     pass 2: (n3, m1):              16-point over n2, times w_256^(m2 n3)   (in place)
+//     pass 3: (m2, m1):              16-point over n3
+// Shared-memory layout idx(n3, r, m1) = n3 * 513 + r * 32 + m1 (r = n2, then m2): every access
+// of every pass is bank-conflict free, and a thread's 32 outputs m = t + 256 s are exactly its
+// 32 inputs of the next transform, so G never leaves the registers.
 #include "bfly_internal.cuh"
+
 namespace bfly {
+
+namespace {
+
+constexpr int NT = 256;            // threads per CTA
+constexpr int PTS = 32;            // points per thread
+constexpr int ROW = 513;           // padded row (n3) stride of the work buffer, in complex
+constexpr int WORK = 16 * ROW;     // complex elements of the work buffer
+static_assert(NT * PTS == FFT_B, "geometry");
+
+// cos(2 pi k / 32), k = 0..8
+__device__ __forceinline__ constexpr float cos32(int k)
+{
+    return k == 0 ? 1.0f
+         : k == 1 ? 0.98078528040323044913f
+         : k == 2 ? 0.92387953251128675613f
+         : k == 3 ? 0.83146961230254523708f
+         : k == 4 ? 0.70710678118654752440f
+         : k == 5 ? 0.55557023301960222474f
+         : k == 6 ? 0.38268343236508977173f
+         : k == 7 ? 0.19509032201612826785f
+         : 0.0f;
+}
+// exp(+2 pi i k / 32) for 0 <= k < 16
+__device__ __forceinline__ constexpr float tw32_re(int k) { return k <= 8 ? cos32(k) : -cos32(16 - k); }
+__device__ __forceinline__ constexpr float tw32_im(int k) { return k <= 8 ? cos32(8 - k) : cos32(k - 8); }
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{
+    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+
+template <int N> __device__ __forceinline__ constexpr int bitrev(int m)
+{
+    int r = 0;
+    for (int b = 1; b < N; b <<= 1) { r = (r << 1) | (m & 1); m >>= 1; }
+    return r;
+}
+
+// In-register radix-2 decimation-in-frequency transform Y[m] = sum_n a[n] exp(+2 pi i m n / N);
+// on return a[bitrev(m)] holds Y[m].  Fully unrolled: every index and twiddle is a constant.
+template <int N> __device__ __forceinline__ void fft_dif(float2 (&a)[N])
+{
+#pragma unroll
+    for (int span = N / 2; span >= 1; span >>= 1) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            if ((i & span) == 0) {
+                const int j = i + span;
+                const int k = (i & (span - 1)) * (16 / span);   // twiddle exp(2 pi i k / 32)
+                const float2 u = a[i], v = a[j];
+                a[i] = make_float2(u.x + v.x, u.y + v.y);
+                const float dx = u.x - v.x, dy = u.y - v.y;
+                if (k == 0) {
+                    a[j] = make_float2(dx, dy);
+                } else if (k == 8) {            // times +i
+                    a[j] = make_float2(-dy, dx);
+                } else if (k == 4) {            // times (1 + i)/sqrt 2
+                    a[j] = make_float2((dx - dy) * cos32(4), (dx + dy) * cos32(4));
+                } else if (k == 12) {           // times (-1 + i)/sqrt 2
+                    a[j] = make_float2((-dx - dy) * cos32(4), (dx - dy) * cos32(4));
+                } else {
+                    const float c = tw32_re(k), s = tw32_im(k);
+                    a[j] = make_float2(fmaf(dx, c, -dy * s), fmaf(dx, s, dy * c));
+                }
+            }
+        }
+    }
+}
+
+// The three passes.  In: v[s] = y[t + 256 s].  Out: v[s] = Y[t + 256 s].  `wb` = exp(2 pi i t / 8192).
+// `work` is the CTA's shared work buffer, `tw256` the shared table exp(2 pi i k / 256).
+__device__ __forceinline__ void fft8192(float2 (&v)[PTS], float2 *__restrict__ work,
+                                        const float2 *__restrict__ tw256, const float2 wb, const int t)
+{
+    // ---- pass 1: 32-point over n1, twiddle w_8192^(m1 t), store at (n3, n2, m1)
+    fft_dif<32>(v);
+    {
+        const float2 w2 = cmul(wb, wb), w3 = cmul(w2, wb), w4 = cmul(w2, w2);
+        float2 ch[4] = {w4, wb, w2, w3};
+        float2 *dst = work + (t & 15) * ROW + (t >> 4) * 32;
+        __syncthreads();                       // the previous transform's pass-3 reads are done
+        dst[0] = v[0];
+#pragma unroll
+        for (int m1 = 1; m1 < 32; ++m1) {
+            if (m1 > 4) ch[m1 & 3] = cmul(ch[m1 & 3], w4);
+            dst[m1] = cmul(v[bitrev<32>(m1)], ch[m1 & 3]);
+        }
+    }
+    __syncthreads();
+    // ---- pass 2: 16-point over n2, twiddle w_256^(m2 n3), in place
+#pragma unroll
+    for (int bf = 0; bf < 2; ++bf) {
+        const int q = t + NT * bf, n3 = q >> 5, m1 = q & 31;
+        float2 *p = work + n3 * ROW + m1;
+        float2 a[16];
+#pragma unroll
+        for (int n2 = 0; n2 < 16; ++n2) a[n2] = p[n2 * 32];
+        fft_dif<16>(a);
+        p[0] = a[0];
+#pragma unroll
+        for (int m2 = 1; m2 < 16; ++m2) p[m2 * 32] = cmul(a[bitrev<16>(m2)], tw256[(m2 * n3) & 255]);
+    }
+    __syncthreads();
+    // ---- pass 3: 16-point over n3; output m = q + 512 m3 lands in slot 2 m3 + bf
+#pragma unroll
+    for (int bf = 0; bf < 2; ++bf) {
+        const float2 *p = work + t + NT * bf;
+        float2 a[16];
+#pragma unroll
+        for (int n3 = 0; n3 < 16; ++n3) a[n3] = p[n3 * ROW];
+        fft_dif<16>(a);
+#pragma unroll
+        for (int m3 = 0; m3 < 16; ++m3) v[2 * m3 + bf] = a[bitrev<16>(m3)];
+    }
+}
+
+__device__ __forceinline__ void fill_tw256(float2 *tw256, int t)
+{
+    float s, c;
+    sincospif((float)t * (1.0f / 128.0f), &s, &c);
+    tw256[t] = make_float2(c, s);
+}
+
+// X_b = conj(F+(xb)) / B for every data block of the call, natural order.
+__global__ void __launch_bounds__(NT, 1)
+data_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_begin, int32_t V,
+                    float2 *__restrict__ xspec)
+{
+    extern __shared__ float2 smem[];
+    float2 *work = smem, *tw256 = smem + WORK;
+    const int t = threadIdx.x;
+    fill_tw256(tw256, t);
+    float2 wb;
+    sincospif((float)t * (1.0f / 4096.0f), &wb.y, &wb.x);
+    const int64_t off = lag_begin + (int64_t)blockIdx.x * V;
+    float2 v[PTS];
+#pragma unroll
+    for (int s = 0; s < PTS; ++s) {
+        const int64_t g = off + t + NT * s;
+        v[s] = make_float2(g < n_samples ? __ldg(x + g) : 0.0f, 0.0f);
+    }
+    fft8192(v, work, tw256, wb, t);
+    float2 *out = xspec + (int64_t)blockIdx.x * FFT_B + t;
+    const float sc = 1.0f / (float)FFT_B;
+#pragma unroll
+    for (int s = 0; s < PTS; ++s) out[NT * s] = make_float2(v[s].x * sc, -v[s].y * sc);
+}
+
+// One CTA per template at a time (persistent, strided over the bank): G = F+(g) in registers,
+// then per data block z = F+(X_b . G) and the fused epilogue (A5-A7).
+__global__ void __launch_bounds__(NT, 1)
+fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
+                     const uint64_t *__restrict__ phB, const float *__restrict__ inc2,
+                     const float *__restrict__ ins2, const float2 *__restrict__ xspec,
+                     const float *__restrict__ rn2, int64_t lag_begin, int64_t n_lags, int32_t V,
+                     int32_t n_blocks, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
+{
+    extern __shared__ float2 smem[];
+    float2 *work = smem, *tw256 = smem + WORK;
+    __shared__ unsigned long long red[NT / 32];
+    const int t = threadIdx.x;
+    fill_tw256(tw256, t);
+    float2 wb;
+    sincospif((float)t * (1.0f / 4096.0f), &wb.y, &wb.x);
+
+    for (int64_t j = blockIdx.x; j < T; j += gridDim.x) {
+        // ---- A3: synthesise g[n] = exp(-i phi_n), n = t + 256 s < L, and transform it
+        const uint64_t A = phA[j], Bq = phB[j];
+        float2 G[PTS];
+#pragma unroll
+        for (int s = 0; s < PTS; ++s) {
+            const int n = t + NT * s;
+            float sn = 0.0f, cs = 0.0f;
+            if (n < L) template_sincos(A, Bq, (uint32_t)n, &sn, &cs);
+            G[s] = make_float2(cs, -sn);
+        }
+        fft8192(G, work, tw256, wb, t);
+        const float ic = inc2[j], is = ins2[j];
+
+        float best = -1.0f;                    // rho^2 >= 0: the first valid lag always wins
+        int32_t best_i = 0;                    // lag index relative to lag_begin
+        for (int32_t b = 0; b < n_blocks; ++b) {
+            // ---- A4: z = F+(X_b . G)
+            const float2 *xb = xspec + (int64_t)b * FFT_B + t;
+            float2 v[PTS];
+#pragma unroll
+            for (int s = 0; s < PTS; ++s) v[s] = __ldg(xb + NT * s);
+#pragma unroll
+            for (int s = 0; s < PTS; ++s) v[s] = cmul(v[s], G[s]);
+            fft8192(v, work, tw256, wb, t);
+            // ---- A5-A7: tau' = t + 256 s; valid while tau' < V and the lag exists
+            const int64_t i0 = (int64_t)b * V;
+            const int64_t left = n_lags - i0;
+            const int32_t vb = left < V ? (int32_t)left : V;
+            const float *r = rn2 + i0 + t;
+#pragma unroll
+            for (int s = 0; s < PTS; ++s) {
+                const int tp = t + NT * s;
+                if (tp < vb) {
+                    const float q = fmaf(v[s].x * v[s].x, ic, v[s].y * v[s].y * is) * __ldg(r + NT * s);
+                    if (q > best) { best = q; best_i = (int32_t)i0 + tp; }
+                }
+            }
+        }
+        // ---- A7: CTA-wide max with ties to the smallest lag
+        unsigned long long p = 0ull;
+        if (best >= 0.0f)
+            p = ((unsigned long long)__float_as_uint(best) << 32) |
+                (unsigned long long)(0xFFFFFFFFu - (uint32_t)best_i);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long q = __shfl_xor_sync(0xffffffffu, p, o);
+            p = q > p ? q : p;
+        }
+        if ((t & 31) == 0) red[t >> 5] = p;
+        __syncthreads();
+        if (t == 0) {
+#pragma unroll
+            for (int w = 1; w < NT / 32; ++w) p = red[w] > p ? red[w] : p;
+            if (p == 0ull) {                    // no valid lag at all (empty range)
+                rho_max[j] = 0.0f;
+                arg_lag[j] = (int32_t)lag_begin;
+            } else {
+                rho_max[j] = sqrtf(__uint_as_float((uint32_t)(p >> 32)));
+                arg_lag[j] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
+            }
+        }
+        __syncthreads();                        // red[] is reused by the next template
+    }
+}
+
+constexpr size_t FFT_SMEM = sizeof(float2) * (size_t)(WORK + 256);
+
+}  // namespace
+
 int64_t fft_blocks_needed(int32_t L, int64_t n_lags)
 {
     const int64_t V = FFT_B - L + 1;
     return n_lags > 0 ? (n_lags + V - 1) / V : 0;
 }
+
 int launch_fft(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream)
 {
-    return launch_direct(b, x, n_samples, lag_begin, lag_end, rho_max, arg_lag, stream);
+    static bool attr_set = false;
+    if (!attr_set) {
+        BFLY_CUDA(cudaFuncSetAttribute(data_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
+        attr_set = true;
+    }
+    const int64_t n_lags = lag_end - lag_begin;
+    const int32_t V = FFT_B - b->L + 1;
+    const int64_t n_blocks = fft_blocks_needed(b->L, n_lags);
+    if (n_blocks * FFT_B > b->xspec_cap) { set_error("FFT workspace too small (internal)"); return BFLY_EINVAL; }
+    if (n_lags >= (1LL << 31)) { set_error("too many lags"); return BFLY_ERANGE; }
+    if (n_blocks > 0) {
+        data_spectra_kernel<<<(unsigned)n_blocks, NT, FFT_SMEM, stream>>>(x, n_samples, lag_begin, V, b->xspec);
+        count_launch();
+        BFLY_CUDA(cudaGetLastError());
+    }
+    const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
+    core_timer_start(b, stream);
+    fft_correlate_kernel<<<(unsigned)ctas, NT, FFT_SMEM, stream>>>(
+        b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, b->xspec, b->rn2, lag_begin, n_lags, V,
+        (int32_t)n_blocks, rho_max, arg_lag);
+    core_timer_stop(b, stream);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    return BFLY_OK;
 }
-}
+
+}  // namespace bfly

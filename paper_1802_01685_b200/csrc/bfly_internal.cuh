@@ -22,8 +22,8 @@ struct bfly_bank {
     // workspace (grown by bfly_bank_reserve / on demand)
     float *rn2;               // 1 / n2[tau] for the lags of the current call
     int64_t rn2_cap;          // floats
-    float2 *xspec;            // data-block spectra, [block][16][512] complex
-    int64_t xspec_cap;        // blocks
+    float2 *xspec;            // data-block spectra X_b, [block][FFT_B] complex, natural order
+    int64_t xspec_cap;        // complex elements
     unsigned long long *packed;  // T packed (rho^2 bits, ~lag) words for the direct form
     float *x_stage;           // device copy of a host chunk (bfly_search_host)
     int64_t x_stage_cap;
