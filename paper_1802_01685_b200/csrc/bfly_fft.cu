@@ -10,26 +10,39 @@
 // X_b is computed once per call by data_spectra_kernel; the correlation kernel keeps G in
 // registers, so per (template, block) the only memory traffic is one read of X_b from L2.
 //
-// The length-8192 transform is 32 x 16 x 16, three passes of register-resident radix-2 DIF
-// butterflies, 256 threads x 32 points:
-//     n = 256 n1 + 16 n2 + n3   ->   m = m1 + 32 m2 + 512 m3
-//     pass 1: thread t = 16 n2 + n3: 32-point over n1, times w_8192^(m1 t)
-//     pass 2: (n3, m1):              16-point over n2, times w_256^(m2 n3)   (in place)
-//     pass 3: (m2, m1):              16-point over n3
-// Shared-memory layout idx(n3, r, m1) = n3 * 513 + r * 32 + m1 (r = n2, then m2): every access
-// of every pass is bank-conflict free, and a thread's 32 outputs m = t + 256 s are exactly its
-// 32 inputs of the next transform, so G never leaves the registers.
+// The length-8192 transform is 16 x 32 x 16, three passes of register-resident radix-2 DIF
+// butterflies, 512 threads x 16 points (16 warps per SM, 128 registers per thread):
+//     n = 512 n1 + 16 n2 + n3   ->   m = m1 + 16 m2 + 512 m3        (n2, m2 < 32; others < 16)
+//     pass 1: thread t = 16 n2 + n3: 16-point over n1, times w_8192^(m1 t)      -> buf0
+//     pass 2: (n3, m1) x role:       32-point over n2 split over a thread pair: role 0 takes
+//             the sums a+b (even m2), role 1 the rotated differences (odd m2); each then runs a
+//             16-point transform; times w_512^(m2 n3)                            buf0 -> buf1
+//     pass 3: thread t = m1 + 16 m2: 16-point over n3                            <- buf1
+// Shared-memory layout idx(n3, r, m1) = n3 * 513 + r * 16 + m1 (r = n2, then m2): every access
+// of every pass is bank-conflict free; the two buffers ping-pong, so a transform needs two
+// __syncthreads; and a thread's 16 outputs m = t + 512 s are exactly its 16 inputs of the next
+// transform, so G never leaves the registers.
 #include "bfly_internal.cuh"
 
 namespace bfly {
 
 namespace {
 
-constexpr int NT = 256;            // threads per CTA
-constexpr int PTS = 32;            // points per thread
-constexpr int ROW = 513;           // padded row (n3) stride of the work buffer, in complex
-constexpr int WORK = 16 * ROW;     // complex elements of the work buffer
+constexpr int NT = 512;            // threads per CTA
+constexpr int PTS = 16;            // points per thread
+constexpr int ROW = 513;           // padded row (n3) stride of a work buffer, in complex
+constexpr int WORK = 16 * ROW;     // complex elements of one work buffer
+constexpr int TW1 = 15 * NT;       // pass 1 -> 2 twiddles w_8192^(m1 t), m1 = 1..15
+constexpr int TW2 = 512;           // pass 2 -> 3 twiddles w_512^k
 static_assert(NT * PTS == FFT_B, "geometry");
+
+struct Smem {                      // carved from dynamic shared memory
+    float2 *buf0, *buf1, *tw1, *tw2;
+};
+__device__ __forceinline__ Smem carve(float2 *base)
+{
+    return Smem{base, base + WORK, base + 2 * WORK, base + 2 * WORK + TW1};
+}
 
 // cos(2 pi k / 32), k = 0..8
 __device__ __forceinline__ constexpr float cos32(int k)
@@ -91,58 +104,71 @@ template <int N> __device__ __forceinline__ void fft_dif(float2 (&a)[N])
     }
 }
 
-// The three passes.  In: v[s] = y[t + 256 s].  Out: v[s] = Y[t + 256 s].  `wb` = exp(2 pi i t / 8192).
-// `work` is the CTA's shared work buffer, `tw256` the shared table exp(2 pi i k / 256).
-__device__ __forceinline__ void fft8192(float2 (&v)[PTS], float2 *__restrict__ work,
-                                        const float2 *__restrict__ tw256, const float2 wb, const int t)
+// The three passes.  In: v[s] = y[t + 512 s].  Out: v[s] = Y[t + 512 s].
+__device__ __forceinline__ void fft8192(float2 (&v)[PTS], const Smem &sm, const int t)
 {
-    // ---- pass 1: 32-point over n1, twiddle w_8192^(m1 t), store at (n3, n2, m1)
-    fft_dif<32>(v);
+    // ---- pass 1: 16-point over n1, twiddle w_8192^(m1 t), store at (n3, n2, m1) of buf0
+    fft_dif<16>(v);
     {
-        const float2 w2 = cmul(wb, wb), w3 = cmul(w2, wb), w4 = cmul(w2, w2);
-        float2 ch[4] = {w4, wb, w2, w3};
-        float2 *dst = work + (t & 15) * ROW + (t >> 4) * 32;
-        __syncthreads();                       // the previous transform's pass-3 reads are done
+        float2 *dst = sm.buf0 + (t & 15) * ROW + (t >> 4) * 16;
+        const float2 *tw = sm.tw1 + t;
         dst[0] = v[0];
 #pragma unroll
-        for (int m1 = 1; m1 < 32; ++m1) {
-            if (m1 > 4) ch[m1 & 3] = cmul(ch[m1 & 3], w4);
-            dst[m1] = cmul(v[bitrev<32>(m1)], ch[m1 & 3]);
+        for (int m1 = 1; m1 < 16; ++m1) dst[m1] = cmul(v[bitrev<16>(m1)], tw[(m1 - 1) * NT]);
+    }
+    __syncthreads();
+    // ---- pass 2: 32-point over n2 as (radix-2 stage split over two threads) + 16-point
+    {
+        const int q = t & 255, role = t >> 8, n3 = q >> 4, m1 = q & 15;
+        const float2 *src = sm.buf0 + n3 * ROW + m1;
+        float2 c[16];
+        if (role == 0) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const float2 a = src[i * 16], b = src[(i + 16) * 16];
+                c[i] = make_float2(a.x + b.x, a.y + b.y);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const float2 a = src[i * 16], b = src[(i + 16) * 16];
+                const float dx = a.x - b.x, dy = a.y - b.y;
+                if (i == 0) c[i] = make_float2(dx, dy);
+                else if (i == 8) c[i] = make_float2(-dy, dx);
+                else c[i] = make_float2(fmaf(dx, tw32_re(i), -dy * tw32_im(i)), fmaf(dx, tw32_im(i), dy * tw32_re(i)));
+            }
         }
+        fft_dif<16>(c);
+        float2 *dst = sm.buf1 + n3 * ROW + role * 16 + m1;          // m2 = 2 k + role
+        const float2 *tw = sm.tw2 + role * n3;                      // (2 k + role) n3 < 512
+#pragma unroll
+        for (int k = 0; k < 16; ++k) dst[k * 32] = cmul(c[bitrev<16>(k)], tw[2 * k * n3]);
     }
     __syncthreads();
-    // ---- pass 2: 16-point over n2, twiddle w_256^(m2 n3), in place
-#pragma unroll
-    for (int bf = 0; bf < 2; ++bf) {
-        const int q = t + NT * bf, n3 = q >> 5, m1 = q & 31;
-        float2 *p = work + n3 * ROW + m1;
+    // ---- pass 3: 16-point over n3; output m = t + 512 m3 lands in slot m3
+    {
+        const float2 *src = sm.buf1 + t;
         float2 a[16];
 #pragma unroll
-        for (int n2 = 0; n2 < 16; ++n2) a[n2] = p[n2 * 32];
-        fft_dif<16>(a);
-        p[0] = a[0];
-#pragma unroll
-        for (int m2 = 1; m2 < 16; ++m2) p[m2 * 32] = cmul(a[bitrev<16>(m2)], tw256[(m2 * n3) & 255]);
-    }
-    __syncthreads();
-    // ---- pass 3: 16-point over n3; output m = q + 512 m3 lands in slot 2 m3 + bf
-#pragma unroll
-    for (int bf = 0; bf < 2; ++bf) {
-        const float2 *p = work + t + NT * bf;
-        float2 a[16];
-#pragma unroll
-        for (int n3 = 0; n3 < 16; ++n3) a[n3] = p[n3 * ROW];
+        for (int n3 = 0; n3 < 16; ++n3) a[n3] = src[n3 * ROW];
         fft_dif<16>(a);
 #pragma unroll
-        for (int m3 = 0; m3 < 16; ++m3) v[2 * m3 + bf] = a[bitrev<16>(m3)];
+        for (int m3 = 0; m3 < 16; ++m3) v[m3] = a[bitrev<16>(m3)];
     }
 }
 
-__device__ __forceinline__ void fill_tw256(float2 *tw256, int t)
+// Twiddle tables, once per CTA (the kernels are persistent).
+__device__ __forceinline__ void fill_tables(const Smem &sm, int t)
 {
     float s, c;
-    sincospif((float)t * (1.0f / 128.0f), &s, &c);
-    tw256[t] = make_float2(c, s);
+    sincospif((float)t * (1.0f / 256.0f), &s, &c);
+    sm.tw2[t] = make_float2(c, s);
+#pragma unroll 1
+    for (int m1 = 1; m1 < 16; ++m1) {
+        sincospif((float)(m1 * t) * (1.0f / 4096.0f), &s, &c);
+        sm.tw1[(m1 - 1) * NT + t] = make_float2(c, s);
+    }
+    __syncthreads();
 }
 
 // X_b = conj(F+(xb)) / B for every data block of the call, natural order.
@@ -151,11 +177,9 @@ data_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_
                     float2 *__restrict__ xspec)
 {
     extern __shared__ float2 smem[];
-    float2 *work = smem, *tw256 = smem + WORK;
+    const Smem sm = carve(smem);
     const int t = threadIdx.x;
-    fill_tw256(tw256, t);
-    float2 wb;
-    sincospif((float)t * (1.0f / 4096.0f), &wb.y, &wb.x);
+    fill_tables(sm, t);
     const int64_t off = lag_begin + (int64_t)blockIdx.x * V;
     float2 v[PTS];
 #pragma unroll
@@ -163,7 +187,7 @@ data_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_
         const int64_t g = off + t + NT * s;
         v[s] = make_float2(g < n_samples ? __ldg(x + g) : 0.0f, 0.0f);
     }
-    fft8192(v, work, tw256, wb, t);
+    fft8192(v, sm, t);
     float2 *out = xspec + (int64_t)blockIdx.x * FFT_B + t;
     const float sc = 1.0f / (float)FFT_B;
 #pragma unroll
@@ -180,15 +204,13 @@ fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                      int32_t n_blocks, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
 {
     extern __shared__ float2 smem[];
-    float2 *work = smem, *tw256 = smem + WORK;
+    const Smem sm = carve(smem);
     __shared__ unsigned long long red[NT / 32];
     const int t = threadIdx.x;
-    fill_tw256(tw256, t);
-    float2 wb;
-    sincospif((float)t * (1.0f / 4096.0f), &wb.y, &wb.x);
+    fill_tables(sm, t);
 
     for (int64_t j = blockIdx.x; j < T; j += gridDim.x) {
-        // ---- A3: synthesise g[n] = exp(-i phi_n), n = t + 256 s < L, and transform it
+        // ---- A3: synthesise g[n] = exp(-i phi_n), n = t + 512 s < L, and transform it
         const uint64_t A = phA[j], Bq = phB[j];
         float2 G[PTS];
 #pragma unroll
@@ -198,7 +220,7 @@ fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             if (n < L) template_sincos(A, Bq, (uint32_t)n, &sn, &cs);
             G[s] = make_float2(cs, -sn);
         }
-        fft8192(G, work, tw256, wb, t);
+        fft8192(G, sm, t);
         const float ic = inc2[j], is = ins2[j];
 
         float best = -1.0f;                    // rho^2 >= 0: the first valid lag always wins
@@ -211,8 +233,8 @@ fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             for (int s = 0; s < PTS; ++s) v[s] = __ldg(xb + NT * s);
 #pragma unroll
             for (int s = 0; s < PTS; ++s) v[s] = cmul(v[s], G[s]);
-            fft8192(v, work, tw256, wb, t);
-            // ---- A5-A7: tau' = t + 256 s; valid while tau' < V and the lag exists
+            fft8192(v, sm, t);
+            // ---- A5-A7: tau' = t + 512 s; valid while tau' < V and the lag exists
             const int64_t i0 = (int64_t)b * V;
             const int64_t left = n_lags - i0;
             const int32_t vb = left < V ? (int32_t)left : V;
@@ -253,7 +275,7 @@ fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
     }
 }
 
-constexpr size_t FFT_SMEM = sizeof(float2) * (size_t)(WORK + 256);
+constexpr size_t FFT_SMEM = sizeof(float2) * (size_t)(2 * WORK + TW1 + TW2);
 
 }  // namespace
 
