@@ -196,6 +196,9 @@ data_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_
 
 // One CTA per template at a time (persistent, strided over the bank): G = F+(g) in registers,
 // then per data block z = F+(X_b . G) and the fused epilogue (A5-A7).
+// SV = ceil(V / 512): output slots s >= SV never hold a valid lag (tau' = t + 512 s >= V), so their
+// butterflies in the last pass and their epilogue are dead code (SV = 9 at L = 4096).
+template <int SV>
 __global__ void __launch_bounds__(NT, 1)
 fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                      const uint64_t *__restrict__ phB, const float *__restrict__ inc2,
@@ -240,7 +243,7 @@ fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             const int32_t vb = left < V ? (int32_t)left : V;
             const float *r = rn2 + i0 + t;
 #pragma unroll
-            for (int s = 0; s < PTS; ++s) {
+            for (int s = 0; s < SV; ++s) {
                 const int tp = t + NT * s;
                 if (tp < vb) {
                     const float q = fmaf(v[s].x * v[s].x, ic, v[s].y * v[s].y * is) * __ldg(r + NT * s);
@@ -291,7 +294,9 @@ int launch_fft(const bfly_bank *b, const float *x, int64_t n_samples, int64_t la
     static bool attr_set = false;
     if (!attr_set) {
         BFLY_CUDA(cudaFuncSetAttribute(data_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
         attr_set = true;
     }
     const int64_t n_lags = lag_end - lag_begin;
@@ -306,9 +311,15 @@ int launch_fft(const bfly_bank *b, const float *x, int64_t n_samples, int64_t la
     }
     const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
     core_timer_start(b, stream);
-    fft_correlate_kernel<<<(unsigned)ctas, NT, FFT_SMEM, stream>>>(
-        b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, b->xspec, b->rn2, lag_begin, n_lags, V,
-        (int32_t)n_blocks, rho_max, arg_lag);
+    const int sv = (V + NT - 1) / NT;
+#define BFLY_FFT_LAUNCH(SV_)                                                                        \
+    fft_correlate_kernel<SV_><<<(unsigned)ctas, NT, FFT_SMEM, stream>>>(                             \
+        b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, b->xspec, b->rn2, lag_begin, n_lags, V,       \
+        (int32_t)n_blocks, rho_max, arg_lag)
+    if (sv <= 9) BFLY_FFT_LAUNCH(9);
+    else if (sv <= 13) BFLY_FFT_LAUNCH(13);
+    else BFLY_FFT_LAUNCH(16);
+#undef BFLY_FFT_LAUNCH
     core_timer_stop(b, stream);
     count_launch();
     BFLY_CUDA(cudaGetLastError());
