@@ -54,10 +54,16 @@ enum {
 
 /* Correlation forms (the core, row A4 of DESIGN.md).  All produce the same quantities. */
 enum {
-    BFLY_FORM_DEFAULT = 0, /* the form bfly_correlate() uses: BFLY_FORM_FFT */
-    BFLY_FORM_FFT = 1,     /* hand-written batched overlap-save FFT correlate (fp32) */
-    BFLY_FORM_DIRECT = 2   /* fp32 CUDA-core time-domain sums; slow cross-check of the core */
+    BFLY_FORM_DEFAULT = 0, /* the form bfly_correlate() uses: BFLY_FORM_FFT_TC */
+    BFLY_FORM_FFT = 1,     /* hand-written batched overlap-save FFT correlate, fp32 CUDA cores */
+    BFLY_FORM_DIRECT = 2,  /* fp32 CUDA-core time-domain sums; slow cross-check of the core */
+    BFLY_FORM_FFT_TC = 3   /* the same overlap-save FFT correlate with the butterflies on the
+                              tensor cores: small DFT matrices x data in fp16, fp32 accumulate,
+                              fp32 twiddles and epilogue.  |d rho| ~ 1e-5 + 5e-5 rho.
+                              Needs L >= BFLY_TC_MIN_L (BFLY_EUNSUPPORTED otherwise); the default
+                              form falls back to BFLY_FORM_FFT for shorter templates */
 };
+#define BFLY_TC_MIN_L 256
 
 const char *bfly_strerror(int status);
 const char *bfly_last_error(void);
@@ -151,6 +157,14 @@ int bfly_search_host(bfly_bank *bank, const float *x_host, int64_t n_samples,
  * two events in milliseconds (BFLY_EINVAL if timing is off or no call was made). */
 int bfly_bank_set_timing(bfly_bank *bank, int enable);
 int bfly_bank_core_ms(bfly_bank *bank, float *ms_out);
+
+/* Diagnostic (tests only): the bare length-8192 transform of BFLY_FORM_FFT_TC,
+ *     z[n] = sum_m y[m] exp(+2 pi i m n / 8192),
+ * on one natural-order input.  y_dev, z_dev: DEVICE, 8192 interleaved complex fp32 each
+ * (16384 floats), caller-owned.  full = 0 computes only n < 4096 (what the correlation uses;
+ * z[4096..] is left untouched), full != 0 all 8192 outputs.  Inputs are rounded to fp16, so
+ * |y| must stay within the fp16 range.  Asynchronous on `stream`. */
+int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream);
 
 /* Number of kernel launches the library has enqueued so far in this process (for bench.py's
  * gpu_launches claim). */

@@ -17,9 +17,9 @@ from . import build as _build
 
 __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
            "butterfly_map", "search_host", "launch_count", "lib_path",
-           "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT"]
+           "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "debug_fft_tc"]
 
-FORM_DEFAULT, FORM_FFT, FORM_DIRECT = 0, 1, 2
+FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC = 0, 1, 2, 3
 
 
 class BflyError(RuntimeError):
@@ -55,11 +55,12 @@ def _load():
                                      vp, vp, vp, vp, vp]
     lib.bfly_bank_set_timing.argtypes = [vp, C.c_int]
     lib.bfly_bank_core_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    lib.bfly_debug_fft_tc.argtypes = [vp, vp, C.c_int, vp]
     lib.bfly_launch_count.argtypes = []
     lib.bfly_launch_count.restype = i64
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
                  "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
-                 "bfly_search_host"):
+                 "bfly_search_host", "bfly_debug_fft_tc"):
         getattr(lib, name).restype = C.c_int
     return lib, path
 
@@ -232,6 +233,17 @@ def search_host(bank: Bank, x_host, chunk_samples: int, kappa: float, samples_pe
                                  m.ctypes.data, cnt.ctypes.data, _stream(bank.device)),
            "bfly_search_host")
     return rho, arg, m, cnt
+
+
+def debug_fft_tc(y: torch.Tensor, full: bool = False) -> torch.Tensor:
+    """bfly_debug_fft_tc: the bare tensor-core transform of FORM_FFT_TC on one complex64[8192]
+    device tensor (tests only).  Returns complex64[8192]; entries n >= 4096 are 0 unless full."""
+    if y.dtype != torch.complex64 or y.numel() != 8192 or not y.is_cuda or not y.is_contiguous():
+        raise TypeError("y must be a contiguous complex64[8192] CUDA tensor")
+    z = torch.zeros_like(y)
+    _check(_lib.bfly_debug_fft_tc(C.c_void_p(y.data_ptr()), C.c_void_p(z.data_ptr()),
+                                  int(bool(full)), _stream(y.device.index)), "bfly_debug_fft_tc")
+    return z
 
 
 def launch_count() -> int:

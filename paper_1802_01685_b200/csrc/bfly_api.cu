@@ -75,7 +75,11 @@ static int reserve_for(bfly_bank *b, int64_t n_samples)
     const int64_t n_lags = n_samples - b->L + 1;
     int rc = grow(&b->rn2, &b->rn2_cap, n_lags);
     if (rc) return rc;
-    return grow(&b->xspec, &b->xspec_cap, fft_blocks_needed(b->L, n_lags) * FFT_B);
+    if ((rc = grow(&b->xspec, &b->xspec_cap, fft_blocks_needed(b->L, n_lags) * FFT_B))) return rc;
+    const int64_t nb = tc_blocks_needed(n_lags);
+    if ((rc = grow(&b->xh, &b->xh_cap, nb * 2 * FFT_B))) return rc;
+    if ((rc = grow(&b->rn2p, &b->rn2p_cap, nb * (FFT_B / 2)))) return rc;
+    return grow(&b->qs, &b->qs_cap, nb);
 }
 
 }  // namespace bfly
@@ -107,6 +111,7 @@ void bfly_free_bank(bfly_bank *b)
     cudaSetDevice(b->device);
     cudaFree(b->f0); cudaFree(b->f1); cudaFree(b->phA); cudaFree(b->phB);
     cudaFree(b->inc2); cudaFree(b->ins2); cudaFree(b->rn2); cudaFree(b->xspec);
+    cudaFree(b->xh); cudaFree(b->rn2p); cudaFree(b->qs);
     cudaFree(b->packed); cudaFree(b->x_stage); cudaFree(b->rho_stage); cudaFree(b->arg_stage);
     cudaFree(b->map_stage); cudaFree(b->cnt_stage);
     if (b->ev_start) cudaEventDestroy(b->ev_start);
@@ -244,8 +249,14 @@ int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int
                   (long long)lag_end, (long long)(n_samples - bank->L + 1));
         return BFLY_EINVAL;
     }
-    if (form == BFLY_FORM_DEFAULT) form = BFLY_FORM_FFT;
-    if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
+    // the tensor-core form needs templates long enough for its fp16 rounding errors to average
+    // out; shorter ones go to the fp32 FFT form
+    if (form == BFLY_FORM_DEFAULT) form = bank->L >= BFLY_TC_MIN_L ? BFLY_FORM_FFT_TC : BFLY_FORM_FFT;
+    if (form == BFLY_FORM_FFT_TC && bank->L < BFLY_TC_MIN_L) {
+        set_error("BFLY_FORM_FFT_TC needs L >= %d (L = %d)", BFLY_TC_MIN_L, bank->L);
+        return BFLY_EUNSUPPORTED;
+    }
+    if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT && form != BFLY_FORM_FFT_TC) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
     bfly_bank *b = const_cast<bfly_bank *>(bank);   // the workspace is mutable state of the bank
     BFLY_CUDA(cudaSetDevice(b->device));
     int rc = reserve_for(b, n_samples);
@@ -255,7 +266,16 @@ int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int
     if (rc) return rc;
     if (form == BFLY_FORM_DIRECT)
         return launch_direct(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
-    return launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    if (form == BFLY_FORM_FFT)
+        return launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    return launch_fft_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+}
+
+int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream)
+{
+    if (!y_dev || !z_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    return launch_debug_fft_tc(reinterpret_cast<const float2 *>(y_dev),
+                               reinterpret_cast<float2 *>(z_dev), full, (cudaStream_t)stream);
 }
 
 int bfly_correlate(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int64_t lag_begin,

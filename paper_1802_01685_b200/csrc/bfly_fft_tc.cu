@@ -1,0 +1,413 @@
+// BFLY_FORM_FFT_TC: batched overlap-save FFT correlate whose butterflies run on the tensor cores
+// (rows A3-A7 of DESIGN.md; the paper's method is FFT correlation).
+//
+// Same mathematics as bfly_fft.cu: with g[k] = exp(-i phi_k) zero-padded to B = 8192,
+//     z_b = F+( X_b . G ),  G = F+(g),  X_b = conj(F+(x_b)) / B,   c = Re z, s = -Im z,
+// but each block yields V = 4096 lags (outputs n < 4096 of the transform; the rows delta >= 8 of
+// the last pass are never computed), and the transform is the four-pass tensor-core FFT of
+// bfly_fft_tc.cuh.  Per (template, block): 4 x 16-byte loads of X_b per thread (fp16, stored by
+// tc_spectra_kernel in the operand layout of the first pass), X_b . G in packed fp16, 512
+// mma.sync, one trip through shared memory, fp32 epilogue.  G lives in shared memory in the
+// same operand layout.  Lags past the last whole block (n_lags mod 4096 <= MAX_TAIL, e.g. the
+// 61441st lag of a 16-s segment) are direct fp32 sums taken while the template is synthesised.
+//
+// Data scaling: every block of x is multiplied by a power of two that puts its rms in [1, 2)
+// (rho is scale invariant), so all intermediates sit well inside the fp16 range; the factor is
+// folded, in float64, into the per-lag normaliser tc_norm_kernel writes.
+#include "bfly_fft32.cuh"
+#include "bfly_fft_tc.cuh"
+
+namespace bfly {
+
+namespace {
+
+using namespace tc;
+
+// ------------------------------------------------------------------------------------------
+// Data-block spectra: X_b = conj(F+(x_b 2^s)) / B by the fp32 transform of bfly_fft32.cuh,
+// rounded to fp16 and scattered into the operand layout.  qs[b] = 2^(-2s) / S16^2.
+__global__ void __launch_bounds__(fft32::NT, 1)
+tc_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_begin,
+                  __half *__restrict__ xh, double *__restrict__ qs)
+{
+    extern __shared__ float2 smem[];
+    __shared__ float esum[fft32::NT / 32];
+    const fft32::Smem sm = fft32::carve(smem);
+    const int t = threadIdx.x;
+    fft32::fill_tables(sm, t);
+    const int64_t off = lag_begin + (int64_t)blockIdx.x * TCV;
+    float2 v[fft32::PTS];
+    float e = 0.0f;
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) {
+        const int64_t gi = off + t + fft32::NT * s;
+        const float xv = gi < n_samples ? __ldg(x + gi) : 0.0f;
+        v[s] = make_float2(xv, 0.0f);
+        e = fmaf(xv, xv, e);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((t & 31) == 0) esum[t >> 5] = e;
+    __syncthreads();
+    float tot = 0.0f;
+#pragma unroll
+    for (int w = 0; w < fft32::NT / 32; ++w) tot += esum[w];      // same order in every thread
+    float sc = 1.0f;
+    if (tot > 0.0f && isfinite(tot)) {
+        int ex;
+        frexpf(sqrtf(tot * (1.0f / (float)FFT_B)), &ex);          // rms = m 2^ex, m in [0.5, 1)
+        sc = ldexpf(1.0f, 1 - ex);
+    }
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) v[s].x *= sc;
+    fft32::fft8192(v, sm, t);
+    __half *out = xh + (int64_t)blockIdx.x * (2 * EXCH_WORDS);
+    const float nb = 1.0f / (float)FFT_B;
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) {
+        int word, half;
+        operand_slot(t + fft32::NT * s, word, half);
+        out[2 * word + half] = __float2half_rn(v[s].x * nb);
+        out[2 * (word + 1) + half] = __float2half_rn(-v[s].y * nb);
+    }
+    if (t == 0) qs[blockIdx.x] = 1.0 / ((double)sc * (double)sc * (double)S16 * (double)S16);
+}
+
+// Per-lag normaliser in the order the epilogue reads it: rn2p[b][thread][2 i + e] belongs to lag
+// b 4096 + (4 w + i) + 64 (2t + e) + 512 g and holds qs[b] / n2 (0 if the window is all zero,
+// -inf past the last lag so that such a slot never wins the maximum).  float64 sums as in A2.
+__global__ void __launch_bounds__(256)
+tc_norm_kernel(const float *__restrict__ x, int32_t L, int64_t lag_begin, int64_t n_fft_lags,
+               const double *__restrict__ qs, float *__restrict__ rn2p, int64_t n_slots)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_slots) return;
+    const int slot = (int)(idx & 7), tid = (int)((idx >> 3) & (NT - 1));
+    const int64_t b = idx >> 12;
+    const int w = tid >> 5, g = (tid >> 2) & 7, t = tid & 3;
+    const int n = (4 * w + (slot >> 1)) + 64 * (2 * t + (slot & 1)) + 512 * g;
+    const int64_t i = b * TCV + n;
+    if (i >= n_fft_lags) { rn2p[idx] = -INFINITY; return; }
+    const float *p = x + lag_begin + i;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int32_t k = 0;
+    for (; k + 4 <= L; k += 4) {
+        const double v0 = (double)__ldg(p + k), v1 = (double)__ldg(p + k + 1);
+        const double v2 = (double)__ldg(p + k + 2), v3 = (double)__ldg(p + k + 3);
+        a0 = fma(v0, v0, a0); a1 = fma(v1, v1, a1); a2 = fma(v2, v2, a2); a3 = fma(v3, v3, a3);
+    }
+    for (; k < L; ++k) { const double v = (double)__ldg(p + k); a0 = fma(v, v, a0); }
+    const double n2 = (a0 + a1) + (a2 + a3);
+    rn2p[idx] = n2 > 0.0 ? (float)(qs[b] / n2) : 0.0f;
+}
+
+// ------------------------------------------------------------------------------------------
+struct TcSmem {
+    uint4 *exch;               // two exchange buffers (ping-pong: one __syncthreads per transform)
+    uint4 *gs;                 // G in the operand layout, fp16
+    uint32_t *w16u;            // [2][3][32]: A fragments of W16 rows 8..15 (G transform only)
+    float *tail;               // [16 warps][2 MAX_TAIL] partial sums of the direct tail lags
+    unsigned long long *red;   // [16]
+};
+constexpr size_t TC_SMEM = 2 * EXCH_WORDS * 4 + EXCH_WORDS * 4 + 2 * 3 * 32 * 4 +
+                           16 * 2 * MAX_TAIL * 4 + 16 * 8;
+__device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
+{
+    TcSmem s;
+    s.exch = reinterpret_cast<uint4 *>(base);
+    s.gs = reinterpret_cast<uint4 *>(base + 2 * EXCH_WORDS * 4);
+    s.w16u = reinterpret_cast<uint32_t *>(base + 3 * EXCH_WORDS * 4);
+    s.tail = reinterpret_cast<float *>(base + 3 * EXCH_WORDS * 4 + 2 * 3 * 32 * 4);
+    s.red = reinterpret_cast<unsigned long long *>(base + 3 * EXCH_WORDS * 4 + 2 * 3 * 32 * 4 +
+                                                   16 * 2 * MAX_TAIL * 4);
+    return s;
+}
+
+// One CTA per template at a time (persistent, strided over the bank).
+__global__ void __launch_bounds__(NT, 1)
+tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
+                    const uint64_t *__restrict__ phB, const float *__restrict__ inc2,
+                    const float *__restrict__ ins2, const uint4 *__restrict__ xh,
+                    const float4 *__restrict__ rn2p, const float *__restrict__ x,
+                    const float *__restrict__ rn2, int64_t lag_begin, int32_t n_blocks,
+                    int32_t n_tail, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const TcSmem sm = carve_tc(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, t = lane & 3;
+    Consts k;
+    make_consts(k, tid);
+    if (w == 0) {
+        uint32_t a[3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            dft_frag(a, 16, S16, 8 + g, 8 * h + 2 * t);
+#pragma unroll
+            for (int q = 0; q < 3; ++q) sm.w16u[(h * 3 + q) * 32 + lane] = a[q];
+        }
+    }
+    __syncthreads();
+    int par = 0;                                       // exchange buffer of the next transform
+    const uint32_t nowu[2][3] = {{0, 0, 0}, {0, 0, 0}};
+
+    for (int64_t j = blockIdx.x; j < T; j += gridDim.x) {
+        // ---- A3: synthesise g[n] = exp(-i phi_n), n = 1024 a + 128 g + 16 c + d' < L, as the
+        //      operand fragments of pass A; direct sums for the tail lags on the way
+        const uint64_t A = phA[j], Bq = phB[j];
+        const float ic = inc2[j], kq = ins2[j] / ic;   // ic > 0: cos phi_0 = 1
+        {
+            uint32_t yr[8], yi[8];
+            float tc_[MAX_TAIL], ts_[MAX_TAIL];
+#pragma unroll
+            for (int r = 0; r < MAX_TAIL; ++r) tc_[r] = ts_[r] = 0.0f;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int c = 4 * (w >> 3) + (u >> 1), dp = (w & 7) + 8 * (u & 1);
+                float cs[2], sn[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int n = 1024 * (2 * t + e) + 128 * g + 16 * c + dp;
+                    cs[e] = sn[e] = 0.0f;
+                    if (n < L) {
+                        template_sincos(A, Bq, (uint32_t)n, &sn[e], &cs[e]);
+#pragma unroll
+                        for (int r = 0; r < MAX_TAIL; ++r) {
+                            if (r >= n_tail) break;
+                            const float xv = __ldg(x + lag_begin + (int64_t)n_blocks * TCV + r + n);
+                            tc_[r] = fmaf(xv, cs[e], tc_[r]);
+                            ts_[r] = fmaf(xv, sn[e], ts_[r]);
+                        }
+                    }
+                }
+                yr[u] = pack_h2(cs[0], cs[1]);
+                yi[u] = pack_h2(-sn[0], -sn[1]);
+            }
+            if (n_tail > 0) {
+#pragma unroll
+                for (int r = 0; r < MAX_TAIL; ++r) {
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        tc_[r] += __shfl_xor_sync(0xffffffffu, tc_[r], o);
+                        ts_[r] += __shfl_xor_sync(0xffffffffu, ts_[r], o);
+                    }
+                    if (lane == 0) {
+                        sm.tail[(w * MAX_TAIL + r) * 2] = tc_[r];
+                        sm.tail[(w * MAX_TAIL + r) * 2 + 1] = ts_[r];
+                    }
+                }
+            }
+            chain1(k, yr, yi, sm.exch + par * (EXCH_WORDS / 4), tid);
+        }
+        __syncthreads();
+        // ---- G = F+(g): all 16 rows of the last pass; G / S16 -> fp16 -> operand layout
+        {
+            uint32_t w16u[2][3];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < 3; ++q) w16u[h][q] = sm.w16u[(h * 3 + q) * 32 + lane];
+            __half *gh = reinterpret_cast<__half *>(sm.gs);
+            const float r16 = 1.0f / S16;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                float2 z[2], zu[2];
+                chain2<true>(k, sm.exch + par * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, w16u);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int m = (4 * w + i) + 64 * (2 * t + e) + 512 * g;
+                    int word, half;
+                    operand_slot(m, word, half);
+                    gh[2 * word + half] = __float2half_rn(z[e].x * r16);
+                    gh[2 * (word + 1) + half] = __float2half_rn(z[e].y * r16);
+                    operand_slot(m + 4096, word, half);
+                    gh[2 * word + half] = __float2half_rn(zu[e].x * r16);
+                    gh[2 * (word + 1) + half] = __float2half_rn(zu[e].y * r16);
+                }
+            }
+        }
+        par ^= 1;
+        __syncthreads();
+
+        float best = -1.0f;
+        int32_t code = 0;                              // 8 b + 2 i + e
+        for (int32_t b = 0; b < n_blocks; ++b) {
+            // ---- A4: Y = X_b . G in packed fp16, straight into the fragments of pass A
+            {
+                uint32_t yr[8], yi[8];
+                const uint4 *xb = xh + ((int64_t)b * 4) * NT + tid;
+#pragma unroll
+                for (int ci = 0; ci < 4; ++ci) {
+                    const uint4 xq = __ldg(xb + ci * NT);
+                    const uint4 gq = sm.gs[ci * NT + tid];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const __half2 xr = as_h2(h ? xq.z : xq.x), xi = as_h2(h ? xq.w : xq.y);
+                        const __half2 gr = as_h2(h ? gq.z : gq.x), gi = as_h2(h ? gq.w : gq.y);
+                        yr[2 * ci + h] = as_u32(__hfma2(__hneg2(xi), gi, __hmul2(xr, gr)));
+                        yi[2 * ci + h] = as_u32(__hfma2(xi, gr, __hmul2(xr, gi)));
+                    }
+                }
+                chain1(k, yr, yi, sm.exch + par * (EXCH_WORDS / 4), tid);
+            }
+            __syncthreads();
+            // ---- passes C, D and A5-A7 on the 8 lags of this thread
+            const float4 *rp = rn2p + ((int64_t)b * NT + tid) * 2;
+            const float4 ra = __ldg(rp), rb = __ldg(rp + 1);
+            const float rr[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                float2 z[2], zu[2];
+                chain2<false>(k, sm.exch + par * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, nowu);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const float q = fmaf(z[e].y * kq, z[e].y, z[e].x * z[e].x) * rr[2 * i + e];
+                    if (q > best) { best = q; code = 8 * b + 2 * i + e; }
+                }
+            }
+            par ^= 1;
+        }
+        // ---- tail lags (direct sums) and the CTA-wide maximum, ties to the smallest lag
+        if (n_tail > 0 && tid < n_tail) {
+            float c = 0.0f, s = 0.0f;
+            for (int ww = 0; ww < 16; ++ww) {
+                c += sm.tail[(ww * MAX_TAIL + tid) * 2];
+                s += sm.tail[(ww * MAX_TAIL + tid) * 2 + 1];
+            }
+            const float q = fmaf(s * kq, s, c * c) * __ldg(rn2 + (int64_t)n_blocks * TCV + tid);
+            if (q > best) { best = q; code = 8 * n_blocks + tid; }
+        }
+        unsigned long long p = 0ull;
+        if (best > 0.0f) {
+            const int bb = code >> 3, sl = code & 7;
+            const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * TCV + (uint32_t)(code - 8 * n_blocks)
+                                               : (uint32_t)bb * TCV + (uint32_t)((4 * w + (sl >> 1)) +
+                                                                                 64 * (2 * t + (sl & 1)) + 512 * g);
+            p = ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long q = __shfl_xor_sync(0xffffffffu, p, o);
+            p = q > p ? q : p;
+        }
+        if (lane == 0) sm.red[w] = p;
+        __syncthreads();
+        if (tid == 0) {
+#pragma unroll
+            for (int ww = 1; ww < 16; ++ww) p = sm.red[ww] > p ? sm.red[ww] : p;
+            if (p == 0ull) {                            // rho = 0 at every lag (or no lag at all)
+                rho_max[j] = 0.0f;
+                arg_lag[j] = (int32_t)lag_begin;
+            } else {
+                rho_max[j] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ic);
+                arg_lag[j] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
+            }
+        }
+        __syncthreads();                                // red[], tail[] are reused by the next template
+    }
+}
+
+// Diagnostic: the bare transform on one natural-order input (bfly_debug_fft_tc).
+__global__ void __launch_bounds__(NT, 1)
+tc_debug_fft_kernel(const float2 *__restrict__ y, float2 *__restrict__ z, int full)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const TcSmem sm = carve_tc(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, t = lane & 3;
+    Consts k;
+    make_consts(k, tid);
+    uint32_t w16u[2][3];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) dft_frag(w16u[h], 16, S16, 8 + g, 8 * h + 2 * t);
+    uint32_t yr[8], yi[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        const int c = 4 * (w >> 3) + (u >> 1), dp = (w & 7) + 8 * (u & 1);
+        const int n0 = 1024 * (2 * t) + 128 * g + 16 * c + dp;
+        const float2 v0 = y[n0], v1 = y[n0 + 1024];
+        yr[u] = pack_h2(v0.x, v1.x);
+        yi[u] = pack_h2(v0.y, v1.y);
+    }
+    chain1(k, yr, yi, sm.exch, tid);
+    __syncthreads();
+    const float r16 = 1.0f / S16;
+    for (int i = 0; i < 4; ++i) {
+        float2 o[2], ou[2];
+        if (full) chain2<true>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
+        else chain2<false>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
+        for (int e = 0; e < 2; ++e) {
+            const int m = (4 * w + i) + 64 * (2 * t + e) + 512 * g;
+            z[m] = make_float2(o[e].x * r16, o[e].y * r16);
+            if (full) z[m + 4096] = make_float2(ou[e].x * r16, ou[e].y * r16);
+        }
+    }
+}
+
+}  // namespace
+
+// Blocks of 4096 lags done by the transform and lags left to the direct tail sums.
+void tc_plan(int64_t n_lags, int64_t *n_blocks, int32_t *n_tail)
+{
+    int64_t nb = n_lags / TCV;
+    int64_t rem = n_lags - nb * TCV;
+    if (rem > MAX_TAIL) { nb += 1; rem = 0; }
+    *n_blocks = nb;
+    *n_tail = (int32_t)rem;
+}
+
+int64_t tc_blocks_needed(int64_t n_lags)
+{
+    int64_t nb; int32_t nt;
+    tc_plan(n_lags, &nb, &nt);
+    return nb;
+}
+
+int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                  int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        BFLY_CUDA(cudaFuncSetAttribute(tc_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        attr_set = true;
+    }
+    const int64_t n_lags = lag_end - lag_begin;
+    if (n_lags >= (1LL << 31) - 2 * TCV) { set_error("too many lags"); return BFLY_ERANGE; }
+    int64_t n_blocks; int32_t n_tail;
+    tc_plan(n_lags, &n_blocks, &n_tail);
+    if (n_blocks * 2 * EXCH_WORDS > b->xh_cap || n_blocks * TCV > b->rn2p_cap) {
+        set_error("FFT workspace too small (internal)");
+        return BFLY_EINVAL;
+    }
+    if (n_blocks > 0) {
+        tc_spectra_kernel<<<(unsigned)n_blocks, fft32::NT, fft32::FFT_SMEM, stream>>>(
+            x, n_samples, lag_begin, b->xh, b->qs);
+        count_launch();
+        BFLY_CUDA(cudaGetLastError());
+        const int64_t n_slots = n_blocks * TCV;
+        tc_norm_kernel<<<(unsigned)((n_slots + 255) / 256), 256, 0, stream>>>(
+            x, b->L, lag_begin, n_lags - n_tail, b->qs, b->rn2p, n_slots);
+        count_launch();
+        BFLY_CUDA(cudaGetLastError());
+    }
+    const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
+    core_timer_start(b, stream);
+    tc_correlate_kernel<<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
+        b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
+        reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
+        rho_max, arg_lag);
+    core_timer_stop(b, stream);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    return BFLY_OK;
+}
+
+int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream)
+{
+    BFLY_CUDA(cudaFuncSetAttribute(tc_debug_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+    tc_debug_fft_kernel<<<1, NT, TC_SMEM, stream>>>(y, z, full);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    return BFLY_OK;
+}
+
+}  // namespace bfly

@@ -1,6 +1,7 @@
 // Internal declarations shared by the translation units of libbfly (not part of the C ABI).
 #pragma once
 
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -24,6 +25,12 @@ struct bfly_bank {
     int64_t rn2_cap;          // floats
     float2 *xspec;            // data-block spectra X_b, [block][FFT_B] complex, natural order
     int64_t xspec_cap;        // complex elements
+    __half *xh;               // BFLY_FORM_FFT_TC: data-block spectra, fp16, operand layout
+    int64_t xh_cap;           // halves (16384 per block)
+    float *rn2p;              // BFLY_FORM_FFT_TC: per-lag normaliser in epilogue order
+    int64_t rn2p_cap;         // floats (4096 per block)
+    double *qs;               // BFLY_FORM_FFT_TC: per-block scale 2^(-2s) / S16^2
+    int64_t qs_cap;
     unsigned long long *packed;  // T packed (rho^2 bits, ~lag) words for the direct form
     float *x_stage;           // device copy of a host chunk (bfly_search_host)
     int64_t x_stage_cap;
@@ -81,6 +88,10 @@ int launch_map(const bfly_bank *b, const float *rho_max, const int32_t *arg_lag,
                int32_t n_fbins, int32_t n_tbins, uint32_t *map, unsigned long long *counters,
                cudaStream_t stream);
 int64_t fft_blocks_needed(int32_t L, int64_t n_lags);
+int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                  int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
+int64_t tc_blocks_needed(int64_t n_lags);
+int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream);
 
 // Template phase in cycles, as a 64-bit fixed-point fraction: phi_k/2pi mod 1 = (A k + B k^2) 2^-64.
 __device__ __forceinline__ void template_sincos(uint64_t A, uint64_t B, uint32_t k, float *s,

@@ -20,7 +20,7 @@ def bfly():
     return b
 
 
-FORMS = [pytest.param(1, id="fft"), pytest.param(2, id="direct")]
+FORMS = [pytest.param(3, id="fft_tc"), pytest.param(1, id="fft"), pytest.param(2, id="direct")]
 
 
 def _run(bfly, form, fs, L, f0, f1, x, lag_begin=0, lag_end=None):
@@ -76,6 +76,12 @@ def test_tiny_injection_on_a_grid_node(bfly, form):
 @pytest.mark.parametrize("fs,L,N", [(2000.0, 2000, 9000), (1000.0, 300, 1500), (4096.0, 4096, 4096),
                                      (4096.0, 4096, 12300), (512.0, 2, 40), (777.0, 1023, 9217)])
 def test_ragged_sizes(bfly, form, fs, L, N):
+    if form == 3 and L < 256:
+        # BFLY_FORM_FFT_TC refuses templates shorter than BFLY_TC_MIN_L; the default form
+        # routes them to the fp32 FFT form
+        with pytest.raises(bfly.BflyError):
+            _run(bfly, form, fs, L, [10.0], [1.0], np.zeros(N, np.float32))
+        form = 0
     rng = np.random.default_rng(int(L + N))
     x = rng.standard_normal(N).astype(np.float32)
     T = 37                                           # not a multiple of any tile
@@ -127,9 +133,35 @@ def test_noise_free_injection_gives_rho_one(bfly):
     x = np.zeros(N)
     x[tau0:tau0 + L] = 3.0 * hc
     x = x.astype(np.float32)
-    for form in (1, 2):
+    # fp32 forms: 1e-4; the tensor-core form rounds its operands to fp16 once per pass and is
+    # held to north_star's tolerance (R1: 2e-4), which at rho = 1 is its worst case
+    for form, tol in ((1, 1e-4), (2, 1e-4), (3, 2e-4)):
         _, rho, arg = _run(bfly, form, fs, L, [700.0], [-210.0], x)
-        assert abs(float(rho[0]) - 1.0) < 1e-4 and int(arg[0]) == tau0
+        assert abs(float(rho[0]) - 1.0) < tol and int(arg[0]) == tau0
+
+
+# ----------------------------------------------------------------- the bare tensor-core transform
+@pytest.mark.parametrize("full", [False, True])
+def test_tensor_core_transform_against_numpy(bfly, full):
+    """bfly_debug_fft_tc: z[n] = sum_m y[m] exp(+2 pi i m n / 8192) against numpy's FFT in
+    float64: every output within 4e-3 of the output rms (fp16 operands: 2^-11 relative per
+    pass), rms error below 1e-3; a unit impulse reproduces the DFT column to fp16 accuracy."""
+    rng = np.random.default_rng(123)
+    y = (rng.standard_normal(8192) + 1j * rng.standard_normal(8192)).astype(np.complex64)
+    z = bfly.debug_fft_tc(torch.from_numpy(y).cuda(), full).cpu().numpy()
+    ref = np.fft.ifft(y.astype(np.complex128)) * 8192
+    n_out = 8192 if full else 4096
+    err = np.abs(z[:n_out] - ref[:n_out])
+    scale = np.sqrt(np.mean(np.abs(ref) ** 2))
+    assert err.max() < 4e-3 * scale and np.sqrt(np.mean(err ** 2)) < 1e-3 * scale
+    if not full:
+        assert np.all(z[4096:] == 0)
+    for m in (0, 1, 17, 1024 + 128 + 16 + 1, 8191):
+        y = np.zeros(8192, np.complex64)
+        y[m] = 1.0
+        z = bfly.debug_fft_tc(torch.from_numpy(y).cuda(), full).cpu().numpy()
+        ref = np.exp(2j * np.pi * m * np.arange(n_out) / 8192)
+        assert np.abs(z[:n_out] - ref).max() < 3e-3
 
 
 # ----------------------------------------------------------------- bank parameters (A1)
@@ -186,9 +218,10 @@ def test_full_bank_config2_is_deterministic_and_matches_sub_bank(bfly):
     rs, as_ = bfly.correlate(sub, xd)
     it = torch.from_numpy(idx).cuda()
     assert torch.equal(rs, r1[it]) and torch.equal(as_, a1[it])
-    # the direct form on the same sub-bank agrees with the FFT form within R1
-    rd, ad = bfly.correlate_form(sub, bfly.FORM_DIRECT, xd)
-    assert float((rd - rs).abs().max()) <= 2e-4
+    # the fp32 FFT form and the direct form on the same sub-bank agree with it within R1
+    for other in (bfly.FORM_FFT, bfly.FORM_DIRECT):
+        rd, ad = bfly.correlate_form(sub, other, xd)
+        assert float((rd - rs).abs().max()) <= 2e-4
 
 
 # ----------------------------------------------------------------- A9: streaming from the host
