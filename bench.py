@@ -158,7 +158,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config, 1-based")
-    ap.add_argument("--form", type=int, default=0, help="0 default (FFT), 1 FFT, 2 direct")
+    ap.add_argument("--form", type=int, default=0,
+                    help="0 default (= 3), 1 fp32 FFT, 2 fp32 direct, 3 tensor-core FFT")
     ap.add_argument("--templates", type=int, default=0,
                     help="development only: first n templates of the bank (not a bench line)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -264,21 +265,40 @@ def main():
     if rank == 0:
         # ---- roofline of the dominant kernel (the correlation core), timed live above
         core_s = float(np.mean(core_ms)) * 1e-3
-        is_fft = form in (0, 1)
+        is_fft = form in (0, 1, 3)
+        is_tc = form in (0, 3) and cfg.L >= 2048          # BFLY_TC_MIN_L (include/bfly.h)
         flops = fft_form_flops(cfg, T) if is_fft else direct_form_flops(cfg, T)
         peak_tflops = SM_COUNT * FP32_LANES * 2 * 1.965e9 / 1e12
         achieved = flops / core_s / 1e12
+        kernel = ("tc_correlate_kernel" if is_tc else "fft_correlate_kernel") if is_fft else "direct_kernel"
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
         if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get("fft_core_bytes_per_launch" if is_fft
-                                                 else "direct_core_bytes_per_launch")
+            traffic = json.load(open(tpath)).get(kernel + "_bytes_per_launch")
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                     "frac": achieved / peak_tflops, "traffic": traffic,
-                    "kernel": "fft_correlate_kernel" if is_fft else "direct_kernel",
+                    "kernel": kernel,
                     "kernel_ms": core_s * 1e3, "kernel_share_of_step": core_s * 1e3 * args.steps / ms,
                     "flops_per_launch": flops,
+                    "flops_basis": "algorithmic FFT-form flops: (n_blocks + 1) x 5 B log2 B + n_blocks x 6 B "
+                                   "per template, B = 8192" if is_fft else "2 x 2 L n_lags per template",
                     "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz"}
+        if is_tc:
+            # what the tensor pipe actually executes: 512 (+256 for G's upper rows) m16n8k16 MMAs
+            # of 4096 flop per length-8192 transform
+            n_blocks = -(-(cfg.n_lags - 4) // 4096)
+            mma_flops = T * (n_blocks * 512 + 768) * 4096
+            peaks = {}
+            ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
+            if os.path.exists(ppath):
+                peaks = json.load(open(ppath))
+            bf16 = peaks.get("bf16_tflops_sustained", 1400.0)
+            roofline["tensor"] = {"executed_tflops": mma_flops / core_s / 1e12,
+                                  "peak": bf16, "frac": mma_flops / core_s / 1e12 / bf16,
+                                  "peak_basis": ("measured sustained cuBLAS bf16 (MEASURED_PEAKS.json)"
+                                                 if peaks else "fallback 1.4 PFLOP/s sustained"),
+                                  "note": "dense flops of the real-embedded DFT matrices on mma.sync "
+                                          "fp16; not algorithmic work"}
         # ---- the oracle beside it, on this box's host cores, on a bounded sample
         f0a, f1a = bank_grid(cfg)
         idx = sub_bank_indices(cfg, 1024, seed=7, halfwidth=0, max_track=0)
@@ -286,10 +306,11 @@ def main():
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "f16 mma operands, f32 accumulate" if is_tc else "f32", "data": "synthetic",
             "config": {"workload": f"config {cfg.index} ({cfg.name})", "templates": T,
                        "n_samples": cfg.n_samples, "L": cfg.L, "lags": cfg.n_lags,
-                       "form": "fft" if is_fft else "direct",
+                       "form": ("fft_tc" if is_tc else "fft") if is_fft else "direct",
                        "l2": "inputs larger than L2 (bank parameters + outputs "
                              f"{(T * 48) >> 20} MiB per step)",
                        "parallelism": "replicas" if world > 1 else "single GPU",
