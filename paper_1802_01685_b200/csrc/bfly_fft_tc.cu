@@ -102,28 +102,86 @@ tc_norm_kernel(const float *__restrict__ x, int32_t L, int64_t lag_begin, int64_
 }
 
 // ------------------------------------------------------------------------------------------
+// Shared memory of tc_correlate_kernel (208 KB of the SM's 227 KB; one CTA per SM).
 struct TcSmem {
-    uint4 *exch;               // two exchange buffers (ping-pong: one __syncthreads per transform)
+    uint4 *exch;               // three exchange buffers, cycled by the block pipeline
     uint4 *gs;                 // G in the operand layout, fp16
+    uint4 *xs;                 // two staging slots for X_b (filled by cp.async.bulk)
+    float *xt;                 // x[first tail lag ..], L + MAX_TAIL - 1 samples at xt_slot(n) (direct tail lags)
     uint32_t *w16u;            // [2][3][32]: A fragments of W16 rows 8..15 (G transform only)
     float *tail;               // [16 warps][2 MAX_TAIL] partial sums of the direct tail lags
     unsigned long long *red;   // [16]
+    unsigned long long *bar;   // mbarriers: [0..2] exchange buffer full, [3..4] X_b slot filled
 };
-constexpr size_t TC_SMEM = 2 * EXCH_WORDS * 4 + EXCH_WORDS * 4 + 2 * 3 * 32 * 4 +
-                           16 * 2 * MAX_TAIL * 4 + 16 * 8;
+constexpr int N_EXCH = 3;
+constexpr size_t OFF_GS = (size_t)N_EXCH * EXCH_WORDS * 4;
+constexpr size_t OFF_XS = OFF_GS + EXCH_WORDS * 4;
+constexpr size_t OFF_XT = OFF_XS + 2 * EXCH_WORDS * 4;
+constexpr size_t OFF_W16U = OFF_XT + (FFT_MAX_L + 32) * 4;
+constexpr size_t OFF_TAIL = OFF_W16U + 2 * 3 * 32 * 4;
+constexpr size_t OFF_RED = OFF_TAIL + 16 * 2 * MAX_TAIL * 4;
+constexpr size_t OFF_BAR = OFF_RED + 16 * 8;
+constexpr size_t TC_SMEM = OFF_BAR + 8 * 8;
 __device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
 {
     TcSmem s;
     s.exch = reinterpret_cast<uint4 *>(base);
-    s.gs = reinterpret_cast<uint4 *>(base + 2 * EXCH_WORDS * 4);
-    s.w16u = reinterpret_cast<uint32_t *>(base + 3 * EXCH_WORDS * 4);
-    s.tail = reinterpret_cast<float *>(base + 3 * EXCH_WORDS * 4 + 2 * 3 * 32 * 4);
-    s.red = reinterpret_cast<unsigned long long *>(base + 3 * EXCH_WORDS * 4 + 2 * 3 * 32 * 4 +
-                                                   16 * 2 * MAX_TAIL * 4);
+    s.gs = reinterpret_cast<uint4 *>(base + OFF_GS);
+    s.xs = reinterpret_cast<uint4 *>(base + OFF_XS);
+    s.xt = reinterpret_cast<float *>(base + OFF_XT);
+    s.w16u = reinterpret_cast<uint32_t *>(base + OFF_W16U);
+    s.tail = reinterpret_cast<float *>(base + OFF_TAIL);
+    s.red = reinterpret_cast<unsigned long long *>(base + OFF_RED);
+    s.bar = reinterpret_cast<unsigned long long *>(base + OFF_BAR);
     return s;
 }
 
-// One CTA per template at a time (persistent, strided over the bank).
+// Index of tail-window sample n in sm.xt: a thread's lanes differ in bits 7-9 (g) and 11-12 (t)
+// of n; folding those into the bank bits makes the reads conflict free.
+__device__ __forceinline__ int xt_slot(int n) { return n ^ ((n >> 7) & 7) ^ (((n >> 11) & 3) << 3); }
+
+// mbarrier / bulk-copy wrappers (PTX ISA: "mbarrier", "cp.async.bulk")
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(void *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, void *bar)
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+
+// One CTA per SM, persistent, strided over the bank; one template at a time.  Per template: g is
+// synthesised and transformed to G (two __syncthreads), then the blocks run as a software
+// pipeline: passes A, B of block b + 1 are issued between the wait for the exchange buffer of
+// block b and passes C, D of block b, so the only synchronisation inside the block loop is a
+// split-phase mbarrier (one arrival per warp) that is normally already complete when waited on.
+// Three exchange buffers make that safe: a warp writing buffer (b + 1) mod 3 has passed
+// "full(b)", so every warp has finished passes A, B of block b and hence passes C, D of block
+// b - 2, the previous user of that buffer.  X_b is staged by one 32 KB cp.async.bulk per block,
+// two blocks ahead, into two slots (the sequence of blocks simply continues across templates).
 __global__ void __launch_bounds__(NT, 1)
 tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const uint64_t *__restrict__ phB, const float *__restrict__ inc2,
@@ -132,7 +190,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const float *__restrict__ rn2, int64_t lag_begin, int32_t n_blocks,
                     int32_t n_tail, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     const TcSmem sm = carve_tc(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, t = lane & 3;
     Consts k;
@@ -146,15 +204,42 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             for (int q = 0; q < 3; ++q) sm.w16u[(h * 3 + q) * 32 + lane] = a[q];
         }
     }
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < N_EXCH; ++i) mbar_init(sm.bar + i, NT / 32);
+        mbar_init(sm.bar + 3, 1);
+        mbar_init(sm.bar + 4, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (n_tail > 0)
+        for (int i = tid; i < L + n_tail - 1; i += NT)
+            sm.xt[xt_slot(i)] = __ldg(x + lag_begin + (int64_t)n_blocks * TCV + i);
     __syncthreads();
-    int par = 0;                                       // exchange buffer of the next transform
+
+    constexpr uint32_t XB_BYTES = EXCH_WORDS * 4;
     const uint32_t nowu[2][3] = {{0, 0, 0}, {0, 0, 0}};
+    // templates of this CTA and the running sequence of its blocks (thread 0 issues the copies)
+    const int64_t my_templates = blockIdx.x < T ? (T - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+    const uint64_t total_blocks = (uint64_t)my_templates * (uint64_t)n_blocks;
+    uint64_t issued = 0;                               // thread 0: X_b copies issued so far
+    int32_t next_b = 0;                                // thread 0: block index of copy `issued`
+    if (tid == 0)
+        for (; issued < 2 && issued < total_blocks; ++issued) {
+            mbar_expect_tx(sm.bar + 3 + (int)issued, XB_BYTES);
+            bulk_load(sm.xs + issued * (EXCH_WORDS / 4), xh + (int64_t)next_b * (EXCH_WORDS / 4), XB_BYTES,
+                      sm.bar + 3 + (int)issued);
+            next_b = next_b + 1 == n_blocks ? 0 : next_b + 1;
+        }
+    uint32_t xcnt = 0;                                 // blocks consumed: slot = xcnt & 1, parity = (xcnt >> 1) & 1
+    int wb = 0, rb = 0;                                // exchange buffer written next / read next
+    uint32_t fpar = 0;                                 // bit i: parity to wait for on "full(i)"
 
     for (int64_t j = blockIdx.x; j < T; j += gridDim.x) {
-        // ---- A3: synthesise g[n] = exp(-i phi_n), n = 1024 a + 128 g + 16 c + d' < L, as the
-        //      operand fragments of pass A; direct sums for the tail lags on the way
+        // ---- A3: synthesise g[n] = cos phi_n - i r sin phi_n, r = ||cos phi|| / ||sin phi||,
+        //      n = 1024 a + 128 g + 16 c + d' < L, as the operand fragments of pass A (so that
+        //      |z|^2 / ||cos phi||^2 is the quadrature sum); direct sums for the tail lags
         const uint64_t A = phA[j], Bq = phB[j];
-        const float ic = inc2[j], kq = ins2[j] / ic;   // ic > 0: cos phi_0 = 1
+        const float ic = inc2[j], rq = sqrtf(ins2[j] / ic);   // ic > 0: cos phi_0 = 1
         {
             uint32_t yr[8], yi[8];
             float tc_[MAX_TAIL], ts_[MAX_TAIL];
@@ -170,12 +255,19 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     cs[e] = sn[e] = 0.0f;
                     if (n < L) {
                         template_sincos(A, Bq, (uint32_t)n, &sn[e], &cs[e]);
+                        sn[e] *= rq;
+                        if (n_tail > 0) {
+                            const float xv = sm.xt[xt_slot(n)];
+                            tc_[0] = fmaf(xv, cs[e], tc_[0]);
+                            ts_[0] = fmaf(xv, sn[e], ts_[0]);
+                            if (n_tail > 1) {
 #pragma unroll
-                        for (int r = 0; r < MAX_TAIL; ++r) {
-                            if (r >= n_tail) break;
-                            const float xv = __ldg(x + lag_begin + (int64_t)n_blocks * TCV + r + n);
-                            tc_[r] = fmaf(xv, cs[e], tc_[r]);
-                            ts_[r] = fmaf(xv, sn[e], ts_[r]);
+                                for (int r = 1; r < MAX_TAIL; ++r) {
+                                    const float xr = r < n_tail ? sm.xt[xt_slot(n + r)] : 0.0f;
+                                    tc_[r] = fmaf(xr, cs[e], tc_[r]);
+                                    ts_[r] = fmaf(xr, sn[e], ts_[r]);
+                                }
+                            }
                         }
                     }
                 }
@@ -196,7 +288,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     }
                 }
             }
-            chain1(k, yr, yi, sm.exch + par * (EXCH_WORDS / 4), tid);
+            chain1(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
         }
         __syncthreads();
         // ---- G = F+(g): all 16 rows of the last pass; G / S16 -> fp16 -> operand layout
@@ -210,61 +302,80 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             const float r16 = 1.0f / S16;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                float2 z[2], zu[2];
-                chain2<true>(k, sm.exch + par * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, w16u);
+                cpair z, zu;
+                chain2<true>(k, sm.exch + wb * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, w16u);
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int m = (4 * w + i) + 64 * (2 * t + e) + 512 * g;
                     int word, half;
                     operand_slot(m, word, half);
-                    gh[2 * word + half] = __float2half_rn(z[e].x * r16);
-                    gh[2 * (word + 1) + half] = __float2half_rn(z[e].y * r16);
+                    gh[2 * word + half] = __float2half_rn((e ? z.r.y : z.r.x) * r16);
+                    gh[2 * (word + 1) + half] = __float2half_rn((e ? z.i.y : z.i.x) * r16);
                     operand_slot(m + 4096, word, half);
-                    gh[2 * word + half] = __float2half_rn(zu[e].x * r16);
-                    gh[2 * (word + 1) + half] = __float2half_rn(zu[e].y * r16);
+                    gh[2 * word + half] = __float2half_rn((e ? zu.r.y : zu.r.x) * r16);
+                    gh[2 * (word + 1) + half] = __float2half_rn((e ? zu.i.y : zu.i.x) * r16);
                 }
             }
         }
-        par ^= 1;
         __syncthreads();
+
+        // ---- A4: passes A, B of one block: Y = X_b . G in packed fp16, straight into the
+        //      fragments of pass A; result to exchange buffer wb; one arrival per warp
+        auto front = [&]() {
+            const int slot = xcnt & 1;
+            mbar_wait(sm.bar + 3 + slot, (xcnt >> 1) & 1);
+            ++xcnt;
+            uint32_t yr[8], yi[8];
+            const uint4 *xb = sm.xs + slot * (EXCH_WORDS / 4) + tid;
+#pragma unroll
+            for (int ci = 0; ci < 4; ++ci) {
+                const uint4 xq = xb[ci * NT];
+                const uint4 gq = sm.gs[ci * NT + tid];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const __half2 xr = as_h2(h ? xq.z : xq.x), xi = as_h2(h ? xq.w : xq.y);
+                    const __half2 gr = as_h2(h ? gq.z : gq.x), gi = as_h2(h ? gq.w : gq.y);
+                    yr[2 * ci + h] = as_u32(__hfma2(__hneg2(xi), gi, __hmul2(xr, gr)));
+                    yi[2 * ci + h] = as_u32(__hfma2(xi, gr, __hmul2(xr, gi)));
+                }
+            }
+            chain1(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sm.bar + wb);
+            wb = wb + 1 == N_EXCH ? 0 : wb + 1;
+        };
 
         float best = -1.0f;
         int32_t code = 0;                              // 8 b + 2 i + e
+        if (n_blocks > 0) front();
         for (int32_t b = 0; b < n_blocks; ++b) {
-            // ---- A4: Y = X_b . G in packed fp16, straight into the fragments of pass A
-            {
-                uint32_t yr[8], yi[8];
-                const uint4 *xb = xh + ((int64_t)b * 4) * NT + tid;
-#pragma unroll
-                for (int ci = 0; ci < 4; ++ci) {
-                    const uint4 xq = __ldg(xb + ci * NT);
-                    const uint4 gq = sm.gs[ci * NT + tid];
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const __half2 xr = as_h2(h ? xq.z : xq.x), xi = as_h2(h ? xq.w : xq.y);
-                        const __half2 gr = as_h2(h ? gq.z : gq.x), gi = as_h2(h ? gq.w : gq.y);
-                        yr[2 * ci + h] = as_u32(__hfma2(__hneg2(xi), gi, __hmul2(xr, gr)));
-                        yi[2 * ci + h] = as_u32(__hfma2(xi, gr, __hmul2(xr, gi)));
-                    }
-                }
-                chain1(k, yr, yi, sm.exch + par * (EXCH_WORDS / 4), tid);
+            mbar_wait(sm.bar + rb, (fpar >> rb) & 1);
+            fpar ^= 1u << rb;
+            // every warp has read the X slot of block b: refill it with the block two ahead
+            if (tid == 0 && issued < total_blocks) {
+                const int slot = (int)(issued & 1);
+                mbar_expect_tx(sm.bar + 3 + slot, XB_BYTES);
+                bulk_load(sm.xs + slot * (EXCH_WORDS / 4), xh + (int64_t)next_b * (EXCH_WORDS / 4), XB_BYTES,
+                          sm.bar + 3 + slot);
+                next_b = next_b + 1 == n_blocks ? 0 : next_b + 1;
+                ++issued;
             }
-            __syncthreads();
+            const uint4 *rbuf = sm.exch + rb * (EXCH_WORDS / 4);
+            rb = rb + 1 == N_EXCH ? 0 : rb + 1;
+            if (b + 1 < n_blocks) front();
             // ---- passes C, D and A5-A7 on the 8 lags of this thread
             const float4 *rp = rn2p + ((int64_t)b * NT + tid) * 2;
-            const float4 ra = __ldg(rp), rb = __ldg(rp + 1);
-            const float rr[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
+            const float4 ra = __ldg(rp), rb4 = __ldg(rp + 1);
+            const float2 rr[4] = {make_float2(ra.x, ra.y), make_float2(ra.z, ra.w),
+                                  make_float2(rb4.x, rb4.y), make_float2(rb4.z, rb4.w)};
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                float2 z[2], zu[2];
-                chain2<false>(k, sm.exch + par * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, nowu);
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const float q = fmaf(z[e].y * kq, z[e].y, z[e].x * z[e].x) * rr[2 * i + e];
-                    if (q > best) { best = q; code = 8 * b + 2 * i + e; }
-                }
+                cpair z, zu;
+                chain2<false>(k, rbuf, 4 * w + i, lane, z, zu, nowu);
+                const float2 q = __fmul2_rn(__ffma2_rn(z.i, z.i, __fmul2_rn(z.r, z.r)), rr[i]);
+                if (q.x > best) { best = q.x; code = 8 * b + 2 * i; }
+                if (q.y > best) { best = q.y; code = 8 * b + 2 * i + 1; }
             }
-            par ^= 1;
         }
         // ---- tail lags (direct sums) and the CTA-wide maximum, ties to the smallest lag
         if (n_tail > 0 && tid < n_tail) {
@@ -273,7 +384,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 c += sm.tail[(ww * MAX_TAIL + tid) * 2];
                 s += sm.tail[(ww * MAX_TAIL + tid) * 2 + 1];
             }
-            const float q = fmaf(s * kq, s, c * c) * __ldg(rn2 + (int64_t)n_blocks * TCV + tid);
+            const float q = fmaf(s, s, c * c) * __ldg(rn2 + (int64_t)n_blocks * TCV + tid);
             if (q > best) { best = q; code = 8 * n_blocks + tid; }
         }
         unsigned long long p = 0ull;
@@ -302,7 +413,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 arg_lag[j] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
             }
         }
-        __syncthreads();                                // red[], tail[] are reused by the next template
+        __syncthreads();                                // red[], tail[], gs, exch are reused by the next template
     }
 }
 
@@ -331,13 +442,13 @@ tc_debug_fft_kernel(const float2 *__restrict__ y, float2 *__restrict__ z, int fu
     __syncthreads();
     const float r16 = 1.0f / S16;
     for (int i = 0; i < 4; ++i) {
-        float2 o[2], ou[2];
+        cpair o, ou;
         if (full) chain2<true>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
         else chain2<false>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
         for (int e = 0; e < 2; ++e) {
             const int m = (4 * w + i) + 64 * (2 * t + e) + 512 * g;
-            z[m] = make_float2(o[e].x * r16, o[e].y * r16);
-            if (full) z[m + 4096] = make_float2(ou[e].x * r16, ou[e].y * r16);
+            z[m] = make_float2((e ? o.r.y : o.r.x) * r16, (e ? o.i.y : o.i.x) * r16);
+            if (full) z[m + 4096] = make_float2((e ? ou.r.y : ou.r.x) * r16, (e ? ou.i.y : ou.i.x) * r16);
         }
     }
 }

@@ -25,7 +25,8 @@
 // Accuracy.  DFT matrices are scaled by S8 / S16 so that every entry is (nearly) an fp16 number
 // (S8 / sqrt 2 is within 2.6e-7, relative, of one; the three irrational entries of W16 within
 // 2.9e-5); the scale is taken out again in the fp32 twiddles and in the epilogue.  Twiddles are
-// applied in fp32 on the fp32 accumulators; data are rounded to fp16 once per pass.
+// applied in fp32 (packed FMUL2 / FFMA2) on the fp32 accumulators; data are rounded to fp16 once
+// per pass.
 #pragma once
 
 #include <cuda_fp16.h>
@@ -50,9 +51,24 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi)
 __device__ __forceinline__ __half2 as_h2(uint32_t w) { return *reinterpret_cast<__half2 *>(&w); }
 __device__ __forceinline__ uint32_t as_u32(__half2 v) { return *reinterpret_cast<uint32_t *>(&v); }
 
-__device__ __forceinline__ float2 cmulf(float2 a, float2 b)
+// Two complex numbers held by component: r = (Re p0, Re p1), i = (Im p0, Im p1).  That is how a
+// thread's MMA accumulator arrives ((d0, d1) and (d2, d3) are aligned register pairs), so the
+// twiddle multiply is four packed fp32 instructions (FMUL2 / FFMA2, sm_100) for two points.
+struct cpair { float2 r, i; };
+__device__ __forceinline__ cpair cmul2(const float (&d)[4], const cpair &w)
 {
-    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+    const float2 dr = make_float2(d[0], d[1]), di = make_float2(d[2], d[3]);
+    cpair p;
+    p.r = __ffma2_rn(make_float2(-di.x, -di.y), w.i, __fmul2_rn(dr, w.r));
+    p.i = __ffma2_rn(di, w.r, __fmul2_rn(dr, w.i));
+    return p;
+}
+__device__ __forceinline__ cpair make_cpair(float2 p0, float2 p1)
+{
+    cpair c;
+    c.r = make_float2(p0.x, p1.x);
+    c.i = make_float2(p0.y, p1.y);
+    return c;
 }
 
 // D = A x B (+ C); A = (a0, a1, a2, a0)
@@ -73,9 +89,9 @@ __device__ __forceinline__ void mma_acc(float (&d)[4], const uint32_t (&a)[3], u
 struct Consts {
     uint32_t w8[3];          // A fragment of S8 * W8 (real-embedded)
     uint32_t w16[2][3];      // A fragments of S16 * W16, rows delta < 8, k-step h (d' = 8 h + ..)
-    float2 twAB[2];          // w_64^(g (2t+e)) / S8:            alpha = g, b = 2t + e
-    float2 twBig[8][2];      // [ci*2+h][e]: w_8192^((2t+e + 8g)(16 c + d')) / S8
-    float2 twC[2][2];        // [h][e]: w_128^((8h + 2t + e) g) / S8:  gamma = g
+    cpair twAB;              // e = 0, 1: w_64^(g (2t+e)) / S8:            alpha = g, b = 2t + e
+    cpair twBig[8];          // [ci*2+h], e = 0, 1: w_8192^((2t+e + 8g)(16 c + d')) / S8
+    cpair twC[2];            // [h], e = 0, 1: w_128^((8h + 2t + e) g) / S8:  gamma = g
 };
 
 // exp(+2 pi i num / den) * scale, num reduced mod den first (den a power of two <= 8192)
@@ -105,17 +121,16 @@ __device__ __forceinline__ void make_consts(Consts &k, int tid)
     dft_frag(k.w16[0], 16, S16, g, 2 * t);
     dft_frag(k.w16[1], 16, S16, g, 8 + 2 * t);
     const float r8 = 1.0f / S8;
+    k.twAB = make_cpair(root(g * (2 * t), 64, r8), root(g * (2 * t + 1), 64, r8));
 #pragma unroll
-    for (int e = 0; e < 2; ++e) {
-        k.twAB[e] = root(g * (2 * t + e), 64, r8);
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            const int c = 4 * (w >> 3) + (u >> 1), dp = (w & 7) + 8 * (u & 1);
-            k.twBig[u][e] = root((2 * t + e + 8 * g) * (16 * c + dp), 8192, r8);
-        }
-#pragma unroll
-        for (int h = 0; h < 2; ++h) k.twC[h][e] = root((8 * h + 2 * t + e) * g, 128, r8);
+    for (int u = 0; u < 8; ++u) {
+        const int c = 4 * (w >> 3) + (u >> 1), dp = (w & 7) + 8 * (u & 1);
+        k.twBig[u] = make_cpair(root((2 * t + 8 * g) * (16 * c + dp), 8192, r8),
+                                root((2 * t + 1 + 8 * g) * (16 * c + dp), 8192, r8));
     }
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+        k.twC[h] = make_cpair(root((8 * h + 2 * t) * g, 128, r8), root((8 * h + 2 * t + 1) * g, 128, r8));
 }
 
 // Byte-free addressing of an exchange buffer, in 16-byte chunks: unit U = alpha + 8 beta owns 32
@@ -130,17 +145,15 @@ __device__ __forceinline__ void chain1(const Consts &k, const uint32_t (&yr)[8],
                                        uint4 *exch, int tid)
 {
     const int w = tid >> 5, g = (tid >> 2) & 7, t = tid & 3;
-    float2 v[8][2];
+    cpair v[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
         float d[4];
         mma_z(d, k.w8, yr[u], yi[u]);                 // alpha = g; b = 2t, 2t+1
-        const float2 p0 = cmulf(make_float2(d[0], d[2]), k.twAB[0]);
-        const float2 p1 = cmulf(make_float2(d[1], d[3]), k.twAB[1]);
+        const cpair p = cmul2(d, k.twAB);
         float f[4];
-        mma_z(f, k.w8, pack_h2(p0.x, p1.x), pack_h2(p0.y, p1.y));   // beta = g; alpha = 2t, 2t+1
-        v[u][0] = cmulf(make_float2(f[0], f[2]), k.twBig[u][0]);
-        v[u][1] = cmulf(make_float2(f[1], f[3]), k.twBig[u][1]);
+        mma_z(f, k.w8, pack_h2(p.r.x, p.r.y), pack_h2(p.i.x, p.i.y));   // beta = g; alpha = 2t, 2t+1
+        v[u] = cmul2(f, k.twBig[u]);
     }
     const int chunk0 = (w & 7) * 4 + 2 * (w >> 3);
 #pragma unroll
@@ -149,42 +162,41 @@ __device__ __forceinline__ void chain1(const Consts &k, const uint32_t (&yr)[8],
 #pragma unroll
         for (int p = 0; p < 2; ++p) {                 // c pair (4 cq + 2 p, + 1): units 4p + h, 4p + 2 + h
             uint4 q;
-            q.x = pack_h2(v[4 * p][e].x, v[4 * p + 2][e].x);
-            q.y = pack_h2(v[4 * p][e].y, v[4 * p + 2][e].y);
-            q.z = pack_h2(v[4 * p + 1][e].x, v[4 * p + 3][e].x);
-            q.w = pack_h2(v[4 * p + 1][e].y, v[4 * p + 3][e].y);
+            q.x = e ? pack_h2(v[4 * p].r.y, v[4 * p + 2].r.y) : pack_h2(v[4 * p].r.x, v[4 * p + 2].r.x);
+            q.y = e ? pack_h2(v[4 * p].i.y, v[4 * p + 2].i.y) : pack_h2(v[4 * p].i.x, v[4 * p + 2].i.x);
+            q.z = e ? pack_h2(v[4 * p + 1].r.y, v[4 * p + 3].r.y) : pack_h2(v[4 * p + 1].r.x, v[4 * p + 3].r.x);
+            q.w = e ? pack_h2(v[4 * p + 1].i.y, v[4 * p + 3].i.y) : pack_h2(v[4 * p + 1].i.x, v[4 * p + 3].i.x);
             exch[exch_chunk(U, chunk0 + p)] = q;
         }
     }
 }
 
-// Passes C and D of unit U = 4 w + i.  Out: z[e] = (delta = g, gamma = 2t + e), times S16; with
-// FULL also zu[e] = (delta = 8 + g, ..) using the extra A fragments w16u.
+// Passes C and D of unit U = 4 w + i.  Out (times S16): z = the two outputs (delta = g,
+// gamma = 2t + e), e = 0, 1, by component; with FULL also zu = (delta = 8 + g, ..) using the
+// extra A fragments w16u.
 template <bool FULL>
 __device__ __forceinline__ void chain2(const Consts &k, const uint4 *exch, int U, int lane,
-                                       float2 (&z)[2], float2 (&zu)[2], const uint32_t (&w16u)[2][3])
+                                       cpair &z, cpair &zu, const uint32_t (&w16u)[2][3])
 {
     const uint4 q = exch[exch_chunk(U, lane)];
     float d0[4], d1[4];
     mma_z(d0, k.w8, q.x, q.y);                        // gamma = g; d' = 2t, 2t+1
     mma_z(d1, k.w8, q.z, q.w);                        // gamma = g; d' = 8 + 2t, + 1
-    const float2 a0 = cmulf(make_float2(d0[0], d0[2]), k.twC[0][0]);
-    const float2 a1 = cmulf(make_float2(d0[1], d0[3]), k.twC[0][1]);
-    const float2 b0 = cmulf(make_float2(d1[0], d1[2]), k.twC[1][0]);
-    const float2 b1 = cmulf(make_float2(d1[1], d1[3]), k.twC[1][1]);
-    const uint32_t r0 = pack_h2(a0.x, a1.x), i0 = pack_h2(a0.y, a1.y);
-    const uint32_t r1 = pack_h2(b0.x, b1.x), i1 = pack_h2(b0.y, b1.y);
+    const cpair a = cmul2(d0, k.twC[0]);
+    const cpair b = cmul2(d1, k.twC[1]);
+    const uint32_t r0 = pack_h2(a.r.x, a.r.y), i0 = pack_h2(a.i.x, a.i.y);
+    const uint32_t r1 = pack_h2(b.r.x, b.r.y), i1 = pack_h2(b.i.x, b.i.y);
     float f[4];
     mma_z(f, k.w16[0], r0, i0);
     mma_acc(f, k.w16[1], r1, i1);
-    z[0] = make_float2(f[0], f[2]);
-    z[1] = make_float2(f[1], f[3]);
+    z.r = make_float2(f[0], f[1]);
+    z.i = make_float2(f[2], f[3]);
     if (FULL) {
         float h[4];
         mma_z(h, w16u[0], r0, i0);
         mma_acc(h, w16u[1], r1, i1);
-        zu[0] = make_float2(h[0], h[2]);
-        zu[1] = make_float2(h[1], h[3]);
+        zu.r = make_float2(h[0], h[1]);
+        zu.i = make_float2(h[2], h[3]);
     }
 }
 
