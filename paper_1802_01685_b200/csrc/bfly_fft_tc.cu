@@ -23,6 +23,17 @@ namespace {
 
 using namespace tc;
 
+// Arithmetic of passes A .. C (bfly_fft_tc.cuh): true = all-fp16 (fp16-accumulate MMAs, half2
+// twiddles), false = fp32 accumulators and twiddles, fp16 operands only.  Measured at config 4:
+// all-fp16 is 1.13x faster (1.34 s against 1.51 s per step) with 2.2x the error (rms |d rho|
+// 2.4e-5 against 1.1e-5, maximum over a few hundred templates 9.7e-5 against 3.6e-5) and loses
+// the noise-free rho = 1 case to the 2e-4 tolerance, so the fp32 variant is the one built.
+#ifndef BFLY_TC_HALF
+#define BFLY_TC_HALF 0
+#endif
+constexpr bool TC_HALF = BFLY_TC_HALF != 0;
+typedef ConstsT<TC_HALF> Consts;
+
 // ------------------------------------------------------------------------------------------
 // Data-block spectra: X_b = conj(F+(x_b 2^s)) / B by the fp32 transform of bfly_fft32.cuh,
 // rounded to fp16 and scattered into the operand layout.  qs[b] = 2^(-2s) / S16^2.
@@ -136,6 +147,20 @@ __device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
     return s;
 }
 
+// cos and sin of the template phase at sample n from the top 32 bits of the fixed-point phase
+// (A n + B n^2) 2^-64 cycles: the two products are taken modulo 2^64 and only their high words
+// kept (error < 2^-31 cycle), the angle goes to the SFU (sin.approx / cos.approx: absolute error
+// ~ 2^-21 on [-pi, pi], far below the fp16 rounding of g that follows).
+__device__ __forceinline__ void synth_sincos(uint32_t Ahi, uint32_t Alo, uint32_t Bhi, uint32_t Blo,
+                                             uint32_t n, float *s, float *c)
+{
+    const uint32_t n2 = n * n;                                   // n < 2^12
+    const uint32_t ph = n * Ahi + __umulhi(n, Alo) + n2 * Bhi + __umulhi(n2, Blo);
+    const float ang = (float)(int32_t)ph * 1.4629180792671596e-9f;   // pi 2^-31: angle in [-pi, pi)
+    *s = __sinf(ang);
+    *c = __cosf(ang);
+}
+
 // Index of tail-window sample n in sm.xt: a thread's lanes differ in bits 7-9 (g) and 11-12 (t)
 // of n; folding those into the bank bits makes the reads conflict free.
 __device__ __forceinline__ int xt_slot(int n) { return n ^ ((n >> 7) & 7) ^ (((n >> 11) & 3) << 3); }
@@ -239,6 +264,8 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         //      n = 1024 a + 128 g + 16 c + d' < L, as the operand fragments of pass A (so that
         //      |z|^2 / ||cos phi||^2 is the quadrature sum); direct sums for the tail lags
         const uint64_t A = phA[j], Bq = phB[j];
+        const uint32_t Ahi = (uint32_t)(A >> 32), Alo = (uint32_t)A;
+        const uint32_t Bhi = (uint32_t)(Bq >> 32), Blo = (uint32_t)Bq;
         const float ic = inc2[j], rq = sqrtf(ins2[j] / ic);   // ic > 0: cos phi_0 = 1
         {
             uint32_t yr[8], yi[8];
@@ -254,7 +281,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const int n = 1024 * (2 * t + e) + 128 * g + 16 * c + dp;
                     cs[e] = sn[e] = 0.0f;
                     if (n < L) {
-                        template_sincos(A, Bq, (uint32_t)n, &sn[e], &cs[e]);
+                        synth_sincos(Ahi, Alo, Bhi, Blo, (uint32_t)n, &sn[e], &cs[e]);
                         sn[e] *= rq;
                         if (n_tail > 0) {
                             const float xv = sm.xt[xt_slot(n)];
@@ -277,6 +304,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             if (n_tail > 0) {
 #pragma unroll
                 for (int r = 0; r < MAX_TAIL; ++r) {
+                    if (r >= n_tail) break;
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) {
                         tc_[r] += __shfl_xor_sync(0xffffffffu, tc_[r], o);
@@ -303,7 +331,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 cpair z, zu;
-                chain2<true>(k, sm.exch + wb * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, w16u);
+                chain2<true, TC_HALF>(k, sm.exch + wb * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, w16u);
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int m = (4 * w + i) + 64 * (2 * t + e) + 512 * g;
@@ -371,7 +399,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 cpair z, zu;
-                chain2<false>(k, rbuf, 4 * w + i, lane, z, zu, nowu);
+                chain2<false, TC_HALF>(k, rbuf, 4 * w + i, lane, z, zu, nowu);
                 const float2 q = __fmul2_rn(__ffma2_rn(z.i, z.i, __fmul2_rn(z.r, z.r)), rr[i]);
                 if (q.x > best) { best = q.x; code = 8 * b + 2 * i; }
                 if (q.y > best) { best = q.y; code = 8 * b + 2 * i + 1; }
@@ -443,8 +471,8 @@ tc_debug_fft_kernel(const float2 *__restrict__ y, float2 *__restrict__ z, int fu
     const float r16 = 1.0f / S16;
     for (int i = 0; i < 4; ++i) {
         cpair o, ou;
-        if (full) chain2<true>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
-        else chain2<false>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
+        if (full) chain2<true, TC_HALF>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
+        else chain2<false, TC_HALF>(k, sm.exch, 4 * w + i, lane, o, ou, w16u);
         for (int e = 0; e < 2; ++e) {
             const int m = (4 * w + i) + 64 * (2 * t + e) + 512 * g;
             z[m] = make_float2((e ? o.r.y : o.r.x) * r16, (e ? o.i.y : o.i.x) * r16);

@@ -71,6 +71,30 @@ __device__ __forceinline__ cpair make_cpair(float2 p0, float2 p1)
     return c;
 }
 
+// The same two complex numbers in fp16: r = (Re p0, Re p1), i = (Im p0, Im p1) as half2 words --
+// the accumulator fragment of an fp16-accumulate MMA and, unchanged, the B fragment of the next.
+struct hpair { uint32_t r, i; };
+__device__ __forceinline__ hpair cmul2(const uint32_t (&d)[2], const hpair &w)
+{
+    const __half2 dr = as_h2(d[0]), di = as_h2(d[1]), wr = as_h2(w.r), wi = as_h2(w.i);
+    hpair p;
+    p.r = as_u32(__hfma2(__hneg2(di), wi, __hmul2(dr, wr)));
+    p.i = as_u32(__hfma2(di, wr, __hmul2(dr, wi)));
+    return p;
+}
+__device__ __forceinline__ hpair make_hpair(float2 p0, float2 p1)
+{
+    hpair c;
+    c.r = pack_h2(p0.x, p1.x);
+    c.i = pack_h2(p0.y, p1.y);
+    return c;
+}
+template <bool HALF> struct TwT { typedef cpair type; };
+template <> struct TwT<true> { typedef hpair type; };
+template <bool HALF> __device__ __forceinline__ typename TwT<HALF>::type make_tw(float2 p0, float2 p1);
+template <> __device__ __forceinline__ cpair make_tw<false>(float2 p0, float2 p1) { return make_cpair(p0, p1); }
+template <> __device__ __forceinline__ hpair make_tw<true>(float2 p0, float2 p1) { return make_hpair(p0, p1); }
+
 // D = A x B (+ C); A = (a0, a1, a2, a0)
 __device__ __forceinline__ void mma_z(float (&d)[4], const uint32_t (&a)[3], uint32_t b0, uint32_t b1)
 {
@@ -85,13 +109,25 @@ __device__ __forceinline__ void mma_acc(float (&d)[4], const uint32_t (&a)[3], u
         : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(b0), "r"(b1));
 }
 
-// Per-thread constants of the transform (registers for the whole kernel).
-struct Consts {
+// fp16-accumulate variant: d0 = (row g, cols 2t, 2t+1), d1 = (row g + 8, ..) as half2 words
+__device__ __forceinline__ void mma_h(uint32_t (&d)[2], const uint32_t (&a)[3], uint32_t b0, uint32_t b1)
+{
+    asm("mma.sync.aligned.m16n8k16.row.col.f16.f16.f16.f16 {%0,%1}, {%2,%3,%4,%2}, {%5,%6}, {%7,%7};"
+        : "=r"(d[0]), "=r"(d[1])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(b0), "r"(b1), "r"(0u));
+}
+
+// Per-thread constants of the transform (registers for the whole kernel).  HALF selects the
+// all-fp16 inner passes (fp16-accumulate MMAs, half2 twiddles: no fp32 <-> fp16 conversions
+// between passes A .. C; pass D and the epilogue stay fp32).
+template <bool HALF>
+struct ConstsT {
     uint32_t w8[3];          // A fragment of S8 * W8 (real-embedded)
     uint32_t w16[2][3];      // A fragments of S16 * W16, rows delta < 8, k-step h (d' = 8 h + ..)
-    cpair twAB;              // e = 0, 1: w_64^(g (2t+e)) / S8:            alpha = g, b = 2t + e
-    cpair twBig[8];          // [ci*2+h], e = 0, 1: w_8192^((2t+e + 8g)(16 c + d')) / S8
-    cpair twC[2];            // [h], e = 0, 1: w_128^((8h + 2t + e) g) / S8:  gamma = g
+    typedef typename TwT<HALF>::type tw_t;
+    tw_t twAB;               // e = 0, 1: w_64^(g (2t+e)) / S8:            alpha = g, b = 2t + e
+    tw_t twBig[8];           // [ci*2+h], e = 0, 1: w_8192^((2t+e + 8g)(16 c + d')) / S8
+    tw_t twC[2];             // [h], e = 0, 1: w_128^((8h + 2t + e) g) / S8:  gamma = g
 };
 
 // exp(+2 pi i num / den) * scale, num reduced mod den first (den a power of two <= 8192)
@@ -114,23 +150,24 @@ __device__ __forceinline__ void dft_frag(uint32_t (&a)[3], int r, float scale, i
 // Warp w handles, before the exchange, the eight 64-point sub-transforms ("units") with
 // c = 4 (w >> 3) + ci, d' = (w & 7) + 8 h  (unit index u = 2 ci + h), and after it the four
 // units with alpha + 8 beta = 4 w + i.
-__device__ __forceinline__ void make_consts(Consts &k, int tid)
+template <bool HALF>
+__device__ __forceinline__ void make_consts(ConstsT<HALF> &k, int tid)
 {
     const int w = tid >> 5, g = (tid >> 2) & 7, t = tid & 3;
     dft_frag(k.w8, 8, S8, g, 2 * t);
     dft_frag(k.w16[0], 16, S16, g, 2 * t);
     dft_frag(k.w16[1], 16, S16, g, 8 + 2 * t);
     const float r8 = 1.0f / S8;
-    k.twAB = make_cpair(root(g * (2 * t), 64, r8), root(g * (2 * t + 1), 64, r8));
+    k.twAB = make_tw<HALF>(root(g * (2 * t), 64, r8), root(g * (2 * t + 1), 64, r8));
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
         const int c = 4 * (w >> 3) + (u >> 1), dp = (w & 7) + 8 * (u & 1);
-        k.twBig[u] = make_cpair(root((2 * t + 8 * g) * (16 * c + dp), 8192, r8),
+        k.twBig[u] = make_tw<HALF>(root((2 * t + 8 * g) * (16 * c + dp), 8192, r8),
                                 root((2 * t + 1 + 8 * g) * (16 * c + dp), 8192, r8));
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h)
-        k.twC[h] = make_cpair(root((8 * h + 2 * t) * g, 128, r8), root((8 * h + 2 * t + 1) * g, 128, r8));
+        k.twC[h] = make_tw<HALF>(root((8 * h + 2 * t) * g, 128, r8), root((8 * h + 2 * t + 1) * g, 128, r8));
 }
 
 // Byte-free addressing of an exchange buffer, in 16-byte chunks: unit U = alpha + 8 beta owns 32
@@ -141,8 +178,8 @@ __device__ __forceinline__ int exch_chunk(int U, int chunk) { return U * 32 + (c
 
 // Passes A and B of the eight units of this warp.  In: yr[u], yi[u] = B fragments (fp16x2 pairs
 // over a = 2t, 2t+1; column b = g).  Out: stored to the exchange buffer.
-__device__ __forceinline__ void chain1(const Consts &k, const uint32_t (&yr)[8], const uint32_t (&yi)[8],
-                                       uint4 *exch, int tid)
+__device__ __forceinline__ void chain1(const ConstsT<false> &k, const uint32_t (&yr)[8],
+                                       const uint32_t (&yi)[8], uint4 *exch, int tid)
 {
     const int w = tid >> 5, g = (tid >> 2) & 7, t = tid & 3;
     cpair v[8];
@@ -171,30 +208,76 @@ __device__ __forceinline__ void chain1(const Consts &k, const uint32_t (&yr)[8],
     }
 }
 
+__device__ __forceinline__ void chain1(const ConstsT<true> &k, const uint32_t (&yr)[8],
+                                       const uint32_t (&yi)[8], uint4 *exch, int tid)
+{
+    const int w = tid >> 5, g = (tid >> 2) & 7, t = tid & 3;
+    hpair v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        uint32_t d[2], f[2];
+        mma_h(d, k.w8, yr[u], yi[u]);                 // alpha = g; b = 2t, 2t+1
+        const hpair p = cmul2(d, k.twAB);
+        mma_h(f, k.w8, p.r, p.i);                     // beta = g; alpha = 2t, 2t+1
+        v[u] = cmul2(f, k.twBig[u]);
+    }
+    const int chunk0 = (w & 7) * 4 + 2 * (w >> 3);
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        const int U = 2 * t + e + 8 * g;
+        const uint32_t sel = e ? 0x7632u : 0x5410u;   // the e-th halves of two words
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {                 // c pair (4 cq + 2 p, + 1): units 4p + h, 4p + 2 + h
+            uint4 q;
+            q.x = __byte_perm(v[4 * p].r, v[4 * p + 2].r, sel);
+            q.y = __byte_perm(v[4 * p].i, v[4 * p + 2].i, sel);
+            q.z = __byte_perm(v[4 * p + 1].r, v[4 * p + 3].r, sel);
+            q.w = __byte_perm(v[4 * p + 1].i, v[4 * p + 3].i, sel);
+            exch[exch_chunk(U, chunk0 + p)] = q;
+        }
+    }
+}
+
 // Passes C and D of unit U = 4 w + i.  Out (times S16): z = the two outputs (delta = g,
 // gamma = 2t + e), e = 0, 1, by component; with FULL also zu = (delta = 8 + g, ..) using the
 // extra A fragments w16u.
-template <bool FULL>
-__device__ __forceinline__ void chain2(const Consts &k, const uint4 *exch, int U, int lane,
-                                       cpair &z, cpair &zu, const uint32_t (&w16u)[2][3])
+// Pass C of one unit in either arithmetic: the four B-fragment words of pass D.
+__device__ __forceinline__ void pass_c(const ConstsT<false> &k, const uint4 &q, uint32_t (&o)[4])
 {
-    const uint4 q = exch[exch_chunk(U, lane)];
     float d0[4], d1[4];
     mma_z(d0, k.w8, q.x, q.y);                        // gamma = g; d' = 2t, 2t+1
     mma_z(d1, k.w8, q.z, q.w);                        // gamma = g; d' = 8 + 2t, + 1
     const cpair a = cmul2(d0, k.twC[0]);
     const cpair b = cmul2(d1, k.twC[1]);
-    const uint32_t r0 = pack_h2(a.r.x, a.r.y), i0 = pack_h2(a.i.x, a.i.y);
-    const uint32_t r1 = pack_h2(b.r.x, b.r.y), i1 = pack_h2(b.i.x, b.i.y);
+    o[0] = pack_h2(a.r.x, a.r.y); o[1] = pack_h2(a.i.x, a.i.y);
+    o[2] = pack_h2(b.r.x, b.r.y); o[3] = pack_h2(b.i.x, b.i.y);
+}
+__device__ __forceinline__ void pass_c(const ConstsT<true> &k, const uint4 &q, uint32_t (&o)[4])
+{
+    uint32_t d0[2], d1[2];
+    mma_h(d0, k.w8, q.x, q.y);
+    mma_h(d1, k.w8, q.z, q.w);
+    const hpair a = cmul2(d0, k.twC[0]);
+    const hpair b = cmul2(d1, k.twC[1]);
+    o[0] = a.r; o[1] = a.i; o[2] = b.r; o[3] = b.i;
+}
+
+template <bool FULL, bool HALF>
+__device__ __forceinline__ void chain2(const ConstsT<HALF> &k, const uint4 *exch, int U, int lane,
+                                       cpair &z, cpair &zu, const uint32_t (&w16u)[2][3])
+{
+    const uint4 q = exch[exch_chunk(U, lane)];
+    uint32_t o[4];
+    pass_c(k, q, o);
     float f[4];
-    mma_z(f, k.w16[0], r0, i0);
-    mma_acc(f, k.w16[1], r1, i1);
+    mma_z(f, k.w16[0], o[0], o[1]);
+    mma_acc(f, k.w16[1], o[2], o[3]);
     z.r = make_float2(f[0], f[1]);
     z.i = make_float2(f[2], f[3]);
     if (FULL) {
         float h[4];
-        mma_z(h, w16u[0], r0, i0);
-        mma_acc(h, w16u[1], r1, i1);
+        mma_z(h, w16u[0], o[0], o[1]);
+        mma_acc(h, w16u[1], o[2], o[3]);
         zu.r = make_float2(h[0], h[1]);
         zu.i = make_float2(h[2], h[3]);
     }
