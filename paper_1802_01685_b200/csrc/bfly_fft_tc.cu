@@ -449,7 +449,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 __global__ void __launch_bounds__(NT, 1)
 tc_debug_fft_kernel(const float2 *__restrict__ y, float2 *__restrict__ z, int full)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     const TcSmem sm = carve_tc(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, t = lane & 3;
     Consts k;
