@@ -301,7 +301,7 @@ def main():
                                           "fp16; not algorithmic work"}
         # ---- the oracle beside it, on this box's host cores, on a bounded sample
         f0a, f1a = bank_grid(cfg)
-        idx = sub_bank_indices(cfg, 1024, seed=7, halfwidth=0, max_track=0)
+        idx = sub_bank_indices(cfg, 8192, seed=7, halfwidth=0, max_track=0)
         cv, cn, cs, cores = time_oracle(cfg, x, f0a[idx], f1a[idx], args.cpu_seconds)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
