@@ -159,7 +159,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config, 1-based")
     ap.add_argument("--form", type=int, default=0,
-                    help="0 default (= 3), 1 fp32 FFT, 2 fp32 direct, 3 tensor-core FFT")
+                    help="0 default (= 3), 1 fp32 FFT, 2 fp32 direct, 3 tensor-core FFT, 4 dense tcgen05")
     ap.add_argument("--templates", type=int, default=0,
                     help="development only: first n templates of the bank (not a bench line)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

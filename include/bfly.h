@@ -57,6 +57,12 @@ enum {
     BFLY_FORM_DEFAULT = 0, /* the form bfly_correlate() uses: BFLY_FORM_FFT_TC */
     BFLY_FORM_FFT = 1,     /* hand-written batched overlap-save FFT correlate, fp32 CUDA cores */
     BFLY_FORM_DIRECT = 2,  /* fp32 CUDA-core time-domain sums; slow cross-check of the core */
+    BFLY_FORM_DENSE_TC = 4,/* lagged-data Hankel tile x template tile dense contraction on tcgen05
+                              tensor cores (north_star (3)(a)): templates synthesised into shared
+                              memory, data tiles by TMA, fp16 operands, fp32 accumulators in tensor
+                              memory, epilogue per TMEM lane.  Executes 109x the flops of the FFT
+                              forms: a cross-check and the tensor-pipe measurement, not the default.
+                              Needs L >= BFLY_TC_MIN_L like BFLY_FORM_FFT_TC */
     BFLY_FORM_FFT_TC = 3   /* the same overlap-save FFT correlate with the butterflies on the
                               tensor cores: small DFT matrices x data in fp16, fp32 accumulate,
                               fp32 twiddles and epilogue.  |d rho| ~ 1e-5 + 5e-5 rho.

@@ -17,9 +17,10 @@ from . import build as _build
 
 __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
            "butterfly_map", "search_host", "launch_count", "lib_path",
-           "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "debug_fft_tc"]
+           "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC",
+           "debug_fft_tc"]
 
-FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC = 0, 1, 2, 3
+FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC, FORM_DENSE_TC = 0, 1, 2, 3, 4
 
 
 class BflyError(RuntimeError):

@@ -112,6 +112,7 @@ void bfly_free_bank(bfly_bank *b)
     cudaFree(b->f0); cudaFree(b->f1); cudaFree(b->phA); cudaFree(b->phB);
     cudaFree(b->inc2); cudaFree(b->ins2); cudaFree(b->rn2); cudaFree(b->xspec);
     cudaFree(b->xh); cudaFree(b->rn2p); cudaFree(b->qs);
+    cudaFree(b->ys); cudaFree(b->rn2s); cudaFree(b->maxbits);
     cudaFree(b->packed); cudaFree(b->x_stage); cudaFree(b->rho_stage); cudaFree(b->arg_stage);
     cudaFree(b->map_stage); cudaFree(b->cnt_stage);
     if (b->ev_start) cudaEventDestroy(b->ev_start);
@@ -252,11 +253,11 @@ int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int
     // the tensor-core form needs templates long enough for its fp16 rounding errors to average
     // out; shorter ones go to the fp32 FFT form
     if (form == BFLY_FORM_DEFAULT) form = bank->L >= BFLY_TC_MIN_L ? BFLY_FORM_FFT_TC : BFLY_FORM_FFT;
-    if (form == BFLY_FORM_FFT_TC && bank->L < BFLY_TC_MIN_L) {
-        set_error("BFLY_FORM_FFT_TC needs L >= %d (L = %d)", BFLY_TC_MIN_L, bank->L);
+    if ((form == BFLY_FORM_FFT_TC || form == BFLY_FORM_DENSE_TC) && bank->L < BFLY_TC_MIN_L) {
+        set_error("the fp16-operand forms need L >= %d (L = %d)", BFLY_TC_MIN_L, bank->L);
         return BFLY_EUNSUPPORTED;
     }
-    if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT && form != BFLY_FORM_FFT_TC) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
+    if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT && form != BFLY_FORM_FFT_TC && form != BFLY_FORM_DENSE_TC) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
     bfly_bank *b = const_cast<bfly_bank *>(bank);   // the workspace is mutable state of the bank
     BFLY_CUDA(cudaSetDevice(b->device));
     int rc = reserve_for(b, n_samples);
@@ -266,6 +267,8 @@ int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int
     if (rc) return rc;
     if (form == BFLY_FORM_DIRECT)
         return launch_direct(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    if (form == BFLY_FORM_DENSE_TC)
+        return launch_dense_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
     if (form == BFLY_FORM_FFT)
         return launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
     return launch_fft_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);

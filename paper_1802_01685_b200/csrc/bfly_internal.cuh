@@ -31,6 +31,12 @@ struct bfly_bank {
     int64_t rn2p_cap;         // floats (4096 per block)
     double *qs;               // BFLY_FORM_FFT_TC: per-block scale 2^(-2s) / S16^2
     int64_t qs_cap;
+    __half *ys;               // BFLY_FORM_DENSE_TC: eight shifted fp16 copies of the scaled series
+    int64_t ys_cap;
+    float *rn2s;              // BFLY_FORM_DENSE_TC: 1 / (n2 scale^2), padded to whole lag tiles
+    int64_t rn2s_cap;
+    unsigned int *maxbits;    // BFLY_FORM_DENSE_TC: bits of max |x| of the current call
+    int64_t maxbits_cap;
     unsigned long long *packed;  // T packed (rho^2 bits, ~lag) words for the direct form
     float *x_stage;           // device copy of a host chunk (bfly_search_host)
     int64_t x_stage_cap;
@@ -91,6 +97,8 @@ int64_t fft_blocks_needed(int32_t L, int64_t n_lags);
 int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                   int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int64_t tc_blocks_needed(int64_t n_lags);
+int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin, int64_t lag_end,
+                    float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream);
 
 // Template phase in cycles, as a 64-bit fixed-point fraction: phi_k/2pi mod 1 = (A k + B k^2) 2^-64.

@@ -20,7 +20,8 @@ def bfly():
     return b
 
 
-FORMS = [pytest.param(3, id="fft_tc"), pytest.param(1, id="fft"), pytest.param(2, id="direct")]
+FORMS = [pytest.param(3, id="fft_tc"), pytest.param(1, id="fft"), pytest.param(2, id="direct"),
+         pytest.param(4, id="dense_tc")]
 
 
 def _run(bfly, form, fs, L, f0, f1, x, lag_begin=0, lag_end=None):
@@ -76,9 +77,9 @@ def test_tiny_injection_on_a_grid_node(bfly, form):
 @pytest.mark.parametrize("fs,L,N", [(2000.0, 2000, 9000), (1000.0, 300, 1500), (4096.0, 4096, 4096),
                                      (4096.0, 4096, 12300), (512.0, 2, 40), (777.0, 1023, 9217)])
 def test_ragged_sizes(bfly, form, fs, L, N):
-    if form == 3 and L < 256:
-        # BFLY_FORM_FFT_TC refuses templates shorter than BFLY_TC_MIN_L; the default form
-        # routes them to the fp32 FFT form
+    if form in (3, 4) and L < 256:
+        # the fp16-operand forms refuse templates shorter than BFLY_TC_MIN_L (too few terms for
+        # the operand rounding to average out); the default form routes them to the fp32 FFT form
         with pytest.raises(bfly.BflyError):
             _run(bfly, form, fs, L, [10.0], [1.0], np.zeros(N, np.float32))
         form = 0
@@ -135,7 +136,7 @@ def test_noise_free_injection_gives_rho_one(bfly):
     x = x.astype(np.float32)
     # fp32 forms: 1e-4; the tensor-core form rounds its operands to fp16 once per pass and is
     # held to north_star's tolerance (R1: 2e-4), which at rho = 1 is its worst case
-    for form, tol in ((1, 1e-4), (2, 1e-4), (3, 2e-4)):
+    for form, tol in ((1, 1e-4), (2, 1e-4), (3, 2e-4), (4, 2e-4)):
         _, rho, arg = _run(bfly, form, fs, L, [700.0], [-210.0], x)
         assert abs(float(rho[0]) - 1.0) < tol and int(arg[0]) == tau0
 
@@ -222,6 +223,15 @@ def test_full_bank_config2_is_deterministic_and_matches_sub_bank(bfly):
     for other in (bfly.FORM_FFT, bfly.FORM_DIRECT):
         rd, ad = bfly.correlate_form(sub, other, xd)
         assert float((rd - rs).abs().max()) <= 2e-4
+    # the dense tcgen05 form over the WHOLE bank (65536 templates x 126977 lags, out of the CPU
+    # oracle's reach): an independent implementation of A3-A7 agrees within R1 everywhere, is
+    # deterministic, and its argmax is the same wherever the default form's maximum is clear
+    rd, ad = bfly.correlate_form(full, bfly.FORM_DENSE_TC, xd)
+    rd2, ad2 = bfly.correlate_form(full, bfly.FORM_DENSE_TC, xd)
+    torch.cuda.synchronize()
+    assert torch.equal(rd, rd2) and torch.equal(ad, ad2)
+    assert float((rd - r1).abs().max()) <= 2e-4
+    assert float((ad == a1).float().mean()) > 0.9
 
 
 # ----------------------------------------------------------------- A9: streaming from the host
