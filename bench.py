@@ -266,11 +266,20 @@ def main():
         # ---- roofline of the dominant kernel (the correlation core), timed live above
         core_s = float(np.mean(core_ms)) * 1e-3
         is_fft = form in (0, 1, 3)
-        is_tc = form in (0, 3) and cfg.L >= 2048          # BFLY_TC_MIN_L (include/bfly.h)
+        is_tc = form in (0, 3) and cfg.L >= 256           # BFLY_TC_MIN_L (include/bfly.h)
+        is_dense = form == 4
         flops = fft_form_flops(cfg, T) if is_fft else direct_form_flops(cfg, T)
         peak_tflops = SM_COUNT * FP32_LANES * 2 * 1.965e9 / 1e12
         achieved = flops / core_s / 1e12
-        kernel = ("tc_correlate_kernel" if is_tc else "fft_correlate_kernel") if is_fft else "direct_kernel"
+        kernel = (("tc_correlate_kernel" if is_tc else "fft_correlate_kernel") if is_fft
+                  else "dense_tc_kernel" if is_dense else "direct_kernel")
+        peaks = {}
+        ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(ppath):
+            peaks = json.load(open(ppath))
+        bf16 = peaks.get("bf16_tflops_sustained", 1400.0)
+        bf16_basis = ("measured sustained cuBLAS bf16 (MEASURED_PEAKS.json); fp16 operands run at the same rate"
+                      if peaks else "fallback 1.4 PFLOP/s sustained")
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
         if os.path.exists(tpath):
@@ -283,41 +292,60 @@ def main():
                     "flops_basis": "algorithmic FFT-form flops: (n_blocks + 1) x 5 B log2 B + n_blocks x 6 B "
                                    "per template, B = 8192" if is_fft else "2 x 2 L n_lags per template",
                     "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz"}
+        if is_dense:
+            roofline.update({"bound": "tensor", "peak": bf16, "frac": achieved / bf16, "peak_basis": bf16_basis,
+                             "flops_basis": "2 quadratures x 2 L n_lags flop per template (one pass, fp16 operands)"})
         if is_tc:
             # what the tensor pipe actually executes: 512 (+256 for G's upper rows) m16n8k16 MMAs
             # of 4096 flop per length-8192 transform
             n_blocks = -(-(cfg.n_lags - 4) // 4096)
             mma_flops = T * (n_blocks * 512 + 768) * 4096
-            peaks = {}
-            ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
-            if os.path.exists(ppath):
-                peaks = json.load(open(ppath))
-            bf16 = peaks.get("bf16_tflops_sustained", 1400.0)
             roofline["tensor"] = {"executed_tflops": mma_flops / core_s / 1e12,
                                   "peak": bf16, "frac": mma_flops / core_s / 1e12 / bf16,
-                                  "peak_basis": ("measured sustained cuBLAS bf16 (MEASURED_PEAKS.json)"
-                                                 if peaks else "fallback 1.4 PFLOP/s sustained"),
+                                  "peak_basis": bf16_basis,
                                   "note": "dense flops of the real-embedded DFT matrices on mma.sync "
                                           "fp16; not algorithmic work"}
-        # ---- the oracle beside it, on this box's host cores, on a bounded sample
         f0a, f1a = bank_grid(cfg)
+        # ---- the other tensor-core form beside the chosen one ("chosen by measurement"): the dense
+        #      tcgen05 contraction on the first 4 waves of template tiles (cost is linear in T)
+        other = None
+        if is_tc and form in (0, 3) and not args.templates and not cfg.streaming:
+            nd = min(T, 4 * SM_COUNT * 128)
+            dbank = bfly.make_bank(cfg.fs_hz, cfg.L, f0a[:nd], f1a[:nd], local)
+            dbank.reserve(cfg.n_samples)
+            dbank.set_timing(True)
+            dms = []
+            for i in range(3):
+                bfly.correlate_form(dbank, 4, xd, 0, None, rho[:nd], arg[:nd])
+                if i:
+                    dms.append(dbank.core_ms())
+            dsec = float(np.mean(dms)) * 1e-3
+            dfl = direct_form_flops(cfg, nd)
+            other = {"dense_tc": {"kernel": "dense_tc_kernel", "templates": nd, "kernel_ms": dsec * 1e3,
+                                  "value": correlations_per_step(cfg, nd) / dsec, "unit": UNIT,
+                                  "roofline": {"bound": "tensor", "achieved": dfl / dsec / 1e12, "peak": bf16,
+                                               "unit": "TFLOP/s", "frac": dfl / dsec / 1e12 / bf16,
+                                               "peak_basis": bf16_basis},
+                                  "note": "same rows A3-A7 as a Hankel x template contraction on tcgen05; "
+                                          "109x the flops of the FFT form, hence not the default"}}
+        # ---- the oracle beside it, on this box's host cores, on a bounded sample
         idx = sub_bank_indices(cfg, 8192, seed=7, halfwidth=0, max_track=0)
         cv, cn, cs, cores = time_oracle(cfg, x, f0a[idx], f1a[idx], args.cpu_seconds)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None,
-            "dtype": "f16 mma operands, f32 accumulate" if is_tc else "f32", "data": "synthetic",
+            "dtype": "f16 mma operands, f32 accumulate" if (is_tc or is_dense) else "f32", "data": "synthetic",
             "config": {"workload": f"config {cfg.index} ({cfg.name})", "templates": T,
                        "n_samples": cfg.n_samples, "L": cfg.L, "lags": cfg.n_lags,
-                       "form": ("fft_tc" if is_tc else "fft") if is_fft else "direct",
+                       "form": ("fft_tc" if is_tc else "fft") if is_fft else "dense_tc" if is_dense else "direct",
                        "l2": "inputs larger than L2 (bank parameters + outputs "
                              f"{(T * 48) >> 20} MiB per step)",
                        "parallelism": "replicas" if world > 1 else "single GPU",
                        "bank_build_s": bank_s,
                        "partial_bank_dev_run": bool(args.templates)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline,
+            "roofline": roofline, "other_forms": other,
             "pairs_per_s": world * T * cfg.n_lags * args.steps / (ms * 1e-3),
             "direct_equiv_mac_per_s": world * T * cfg.n_lags * 2 * cfg.L * args.steps / (ms * 1e-3),
             "cpu_baseline": {"value": cv, "unit": UNIT, "cores": cores, "kind": "oracle",
