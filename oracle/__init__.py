@@ -43,6 +43,11 @@ def lib():
                               C.c_double, C.c_double, C.c_int32, C.c_int32,
                               C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
         L.bfo_map.restype = None
+        L.bfo_sigma.argtypes = [fp, C.c_int64, C.c_double, C.c_int, C.c_double, C.c_double]
+        L.bfo_sigma.restype = C.c_double
+        L.bfo_tails.argtypes = [fp, C.c_int64, C.c_double, C.c_int, C.c_int64, dp, dp, C.c_int64,
+                                C.c_int64, C.c_double, dp, C.c_int64, ip, ip, dp, C.c_int]
+        L.bfo_tails.restype = C.c_int64
         L.bfo_max_threads.argtypes = []
         L.bfo_max_threads.restype = C.c_int
         _lib = L
@@ -158,3 +163,42 @@ def butterfly_map(f0, rho_max, arg_lag, kappa, lag_origin, samples_per_tbin, f_l
                   k32, int(lag_origin), int(samples_per_tbin), float(f_lo_hz), float(df_hz),
                   int(n_fbins), int(n_tbins), _p(map_out, C.c_uint32), _p(counters, C.c_uint64))
     return map_out, counters
+
+
+def sigma(x, fs, L, f0, f1):
+    """Reading S1: rms per quadrature of the circular matched-filter output of one template
+    over the whole segment."""
+    x = _f32(x)
+    if len(x) < L:
+        raise ValueError("segment shorter than the template")
+    return float(lib().bfo_sigma(_p(x, C.c_float), len(x), float(fs), int(L), float(f0), float(f1)))
+
+
+def tails(x, fs, L, f0, f1, kappa, lag_begin=0, lag_end=None, capacity=None, n_threads=0):
+    """Readings S1-S3: (sigma float64[T], hit_template int32[n], hit_lag int32[n],
+    hit_rho float64[n], total) with hits = valid lags where sqrt(c^2+s^2)/sigma_j > kappa, in
+    ascending (template, lag) order; n = min(total, capacity)."""
+    x = _f32(x)
+    f0, f1 = _f64(f0), _f64(f1)
+    lag_end = len(x) - L + 1 if lag_end is None else lag_end
+    T = len(f0)
+    sig = np.empty(T, np.float64)
+    if capacity is None:
+        # count first, then size the arrays exactly
+        total = lib().bfo_tails(_p(x, C.c_float), len(x), float(fs), int(L), T, _p(f0, C.c_double),
+                                _p(f1, C.c_double), int(lag_begin), int(lag_end), float(kappa),
+                                _p(sig, C.c_double), 0, None, None, None, int(n_threads))
+        if total < 0:
+            raise ValueError("bad arguments")
+        capacity = int(total)
+    hj = np.empty(max(capacity, 1), np.int32)
+    hl = np.empty(max(capacity, 1), np.int32)
+    hr = np.empty(max(capacity, 1), np.float64)
+    total = lib().bfo_tails(_p(x, C.c_float), len(x), float(fs), int(L), T, _p(f0, C.c_double),
+                            _p(f1, C.c_double), int(lag_begin), int(lag_end), float(kappa),
+                            _p(sig, C.c_double), int(capacity), _p(hj, C.c_int32),
+                            _p(hl, C.c_int32), _p(hr, C.c_double), int(n_threads))
+    if total < 0:
+        raise ValueError("bad arguments")
+    n = int(min(total, capacity))
+    return sig, hj[:n], hl[:n], hr[:n], int(total)

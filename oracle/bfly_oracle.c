@@ -23,7 +23,7 @@
  * P2 noise-free injection, P3 time reversal, P4 direct vs FFT, P5 scale
  * invariance, P6 DFT special case against numpy.fft, P7 Parseval sum, P8 noise
  * expectation 2/L, P9 matched injection in noise, P10 map by brute force,
- * P11 chunking.  Parity unpinned (fixed by DESIGN.md readings only, the paper
+ * P11 chunking; PS1-PS5 for the kappa-sigma tails (bfo_sigma, bfo_tails).  Parity unpinned (fixed by DESIGN.md readings only, the paper
  * being silent): the choice of map coordinates (C10: time = start of the matched
  * window, frequency = f0) and the per-chunk hit semantics of streaming (C11).
  *
@@ -255,6 +255,121 @@ void bfo_map(int64_t n_templates, const double *f0, const double *rho_max, const
         else
             counters[1] += 1;
     }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * The paper's own reduction ("only tails of
+ * butterfly output rho exceeding kappa sigma ... are communicated to the CPU"
+ * "sigma is the standard deviation of the matched filtered output rho, computed in a predictor
+ * step by Parseval's Theorem").  Readings S1-S3:
+ *
+ * S1  The matched-filter output whose spread sigma measures is what the paper's length-N FFT
+ *     correlation of a segment produces: the CIRCULAR correlation of the N-sample segment with
+ *     the unit-norm quadrature templates,
+ *         c~(tau) = sum_k x[(tau+k) mod N] hc[k] / nc,   s~(tau) likewise,   tau = 0 .. N-1,
+ *     and sigma is its root mean square per quadrature (the second moment about zero is what
+ *     Parseval's theorem delivers from the spectra):
+ *         sigma^2 = (1 / (2 N)) sum_tau ( c~(tau)^2 + s~(tau)^2 ).
+ * S2  Tails are taken over the VALID lags only (reading C5), of the un-normalised magnitude:
+ *         rho_sigma(tau) = sqrt(c(tau)^2 + s(tau)^2) / sigma  >  kappa      (strict, C9),
+ *     with c, s the unit-norm-template sums of bfo_rho_at (not divided by ||x_tau||).
+ * S3  sigma == 0 (all-zero segment): no hits.
+ * ------------------------------------------------------------------------------------- */
+
+/* S1, written out in the time domain (N L multiply-adds). */
+double bfo_sigma(const float *x, int64_t n_samples, double fs, int L, double f0, double f1)
+{
+    double *hc = (double *)malloc(sizeof(double) * (size_t)L);
+    double *hs = (double *)malloc(sizeof(double) * (size_t)L);
+    double nc, ns, acc = 0.0;
+    bfo_template(fs, L, f0, f1, hc, hs);
+    bfo_template_norms(L, hc, hs, &nc, &ns);
+    for (int64_t tau = 0; tau < n_samples; ++tau) {
+        double c = 0.0, s = 0.0;
+        for (int k = 0; k < L; ++k) {
+            int64_t i = tau + k;
+            if (i >= n_samples) i -= n_samples;          /* circular: L <= N */
+            double xv = (double)x[i];
+            c += xv * hc[k];
+            s += xv * hs[k];
+        }
+        c = (nc > 0.0) ? c / nc : 0.0;
+        s = (ns > 0.0) ? s / ns : 0.0;
+        acc += c * c + s * s;
+    }
+    free(hc); free(hs);
+    return sqrt(acc / (2.0 * (double)n_samples));
+}
+
+/* S1-S3 for a list of templates.  sigma[j] is always written.  Hits are stored in ascending
+ * (template, lag) order, the first `capacity` of them; the return value is the total number
+ * of hits (which may exceed capacity), or -1 on bad arguments. */
+int64_t bfo_tails(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
+                  const double *f0, const double *f1, int64_t lag_begin, int64_t lag_end,
+                  double kappa, double *sigma, int64_t capacity, int32_t *hit_template,
+                  int32_t *hit_lag, double *hit_rho, int n_threads)
+{
+    if (L < 1 || n_samples < L || lag_begin < 0 || lag_end < lag_begin ||
+        lag_end > n_samples - L + 1)
+        return -1;
+    double *xd = (double *)malloc(sizeof(double) * (size_t)n_samples);
+    for (int64_t i = 0; i < n_samples; ++i) xd[i] = (double)x[i];
+    int64_t *count = (int64_t *)calloc((size_t)n_templates, sizeof(int64_t));
+#ifdef _OPENMP
+    if (n_threads <= 0) n_threads = omp_get_max_threads();
+#else
+    n_threads = 1;
+#endif
+    /* pass 1: sigma and the number of hits of every template */
+#pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads)
+    for (int64_t j = 0; j < n_templates; ++j)
+        sigma[j] = bfo_sigma(x, n_samples, fs, L, f0[j], f1[j]);
+    int64_t total = 0;
+    for (int pass = 0; pass < 2; ++pass) {
+        /* pass 0 counts, pass 1 stores at the offsets the counts give (ascending order) */
+        int64_t *offset = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n_templates + 1));
+        offset[0] = 0;
+        for (int64_t j = 0; j < n_templates; ++j) offset[j + 1] = offset[j] + count[j];
+        total = offset[n_templates];
+#pragma omp parallel num_threads(n_threads)
+        {
+            double *hc = (double *)malloc(sizeof(double) * (size_t)L);
+            double *hs = (double *)malloc(sizeof(double) * (size_t)L);
+            double c[BFO_RUN], s[BFO_RUN];
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t j = 0; j < n_templates; ++j) {
+                double nc, ns;
+                bfo_template(fs, L, f0[j], f1[j], hc, hs);
+                bfo_template_norms(L, hc, hs, &nc, &ns);
+                int64_t n_hit = 0;
+                for (int64_t tau0 = lag_begin; tau0 < lag_end && sigma[j] > 0.0; tau0 += BFO_RUN) {
+                    int n = (int)((lag_end - tau0 < BFO_RUN) ? (lag_end - tau0) : BFO_RUN);
+                    bfo_dots_run(xd, L, hc, hs, tau0, n, c, s);
+                    for (int i = 0; i < n; ++i) {
+                        double cv = (nc > 0.0) ? c[i] / nc : 0.0;
+                        double sv = (ns > 0.0) ? s[i] / ns : 0.0;
+                        double r = sqrt(cv * cv + sv * sv) / sigma[j];
+                        if (r > kappa) {
+                            if (pass == 1) {
+                                int64_t at = offset[j] + n_hit;
+                                if (at < capacity) {
+                                    hit_template[at] = (int32_t)j;
+                                    hit_lag[at] = (int32_t)(tau0 + i);
+                                    hit_rho[at] = r;
+                                }
+                            }
+                            ++n_hit;
+                        }
+                    }
+                }
+                count[j] = n_hit;
+            }
+            free(hc); free(hs);
+        }
+        free(offset);
+    }
+    free(count); free(xd);
+    return total;
 }
 
 int bfo_max_threads(void)
