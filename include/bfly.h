@@ -139,6 +139,38 @@ int bfly_butterfly_map(const bfly_bank *bank,
                        double f_lo_hz, double df_hz, int32_t n_fbins, int32_t n_tbins,
                        uint32_t *map_dev, uint64_t *counters_dev, void *stream);
 
+/* ---- The paper's own reduction: tails of the output above kappa sigma ----------------------
+ * PAPER.md:70 ("only tails of butterfly output rho exceeding kappa sigma ... are communicated to
+ * the CPU"), PAPER.md:120 ("sigma is the standard deviation of the matched filtered output rho,
+ * computed in a predictor step by Parseval's Theorem").  Readings S1-S3 of DESIGN.md:
+ *     sigma_j^2 = (1 / (2 N)) sum_{tau < N} ( c~_j(tau)^2 + s~_j(tau)^2 ),   N = n_samples,
+ * c~, s~ the CIRCULAR correlations of the whole segment x_dev[0 .. N) with the unit-norm
+ * quadrature templates (what a length-N FFT correlation produces; evaluated from spectra by
+ * Parseval's theorem, never in the time domain), and a hit is every valid lag
+ * lag_begin <= tau < lag_end with
+ *     rho_sigma = sqrt(c_j(tau)^2 + s_j(tau)^2) / sigma_j  >  kappa          (strict, fp32),
+ * c, s the sums of bfly_correlate before the division by ||x_tau||.  sigma_j = 0 gives no hits.
+ * Outputs (DEVICE, caller-owned): sigma_dev[T] fp32, overwritten; the hit list
+ * hit_template_dev / hit_lag_dev / hit_rho_dev [capacity] in NO particular order (lags relative
+ * to x_dev[0]); *n_hits_dev (uint64) is INCREMENTED by the number of hits found, which may
+ * exceed capacity: hits are then stored at positions old count .. capacity - 1 only and the
+ * caller sees the overflow from the count (the caller zeroes the counter before the first call
+ * and may chain calls into one list).  Needs L >= BFLY_TC_MIN_L (runs on the tensor-core FFT
+ * form); BFLY_EUNSUPPORTED otherwise.  Asynchronous on `stream`. */
+int bfly_tails(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int64_t lag_begin,
+               int64_t lag_end, float kappa, float *sigma_dev, int64_t capacity,
+               int32_t *hit_template_dev, int32_t *hit_lag_dev, float *hit_rho_dev,
+               uint64_t *n_hits_dev, void *stream);
+
+/* One count per hit of a bfly_tails list at (tbin of lag_origin + hit_lag, fbin of the hit
+ * template's f0): the coordinates and accumulation rules of bfly_butterfly_map, but a template
+ * may contribute many hits per segment (the paper's trajectory map).  n_hits is a
+ * HOST value: the number of list entries to use (at most the list's capacity). */
+int bfly_hits_map(const bfly_bank *bank, const int32_t *hit_template_dev, const int32_t *hit_lag_dev,
+                  int64_t n_hits, int64_t lag_origin, int32_t samples_per_tbin, double f_lo_hz,
+                  double df_hz, int32_t n_fbins, int32_t n_tbins, uint32_t *map_dev,
+                  uint64_t *counters_dev, void *stream);
+
 /* ---- A9 / end-to-end: the whole path on a HOST series ------------------------------------
  * Runs A2-A8 over a HOST series x_host[n_samples] (fp32), cut into chunks of chunk_samples
  * samples with an overlap of L samples (hop = chunk_samples - L): chunk c starts at sample

@@ -18,7 +18,7 @@ from . import build as _build
 __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
            "butterfly_map", "search_host", "launch_count", "lib_path",
            "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC",
-           "debug_fft_tc"]
+           "debug_fft_tc", "tails", "hits_map"]
 
 FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC, FORM_DENSE_TC = 0, 1, 2, 3, 4
 
@@ -52,6 +52,8 @@ def _load():
     lib.bfly_correlate.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
     lib.bfly_correlate_form.argtypes = [vp, C.c_int, vp, i64, i64, i64, vp, vp, vp]
     lib.bfly_butterfly_map.argtypes = [vp, vp, vp, f32, i64, i32, f64, f64, i32, i32, vp, vp, vp]
+    lib.bfly_tails.argtypes = [vp, vp, i64, i64, i64, f32, vp, i64, vp, vp, vp, vp, vp]
+    lib.bfly_hits_map.argtypes = [vp, vp, vp, i64, i64, i32, f64, f64, i32, i32, vp, vp, vp]
     lib.bfly_search_host.argtypes = [vp, vp, i64, i64, f32, i32, f64, f64, i32, i32,
                                      vp, vp, vp, vp, vp]
     lib.bfly_bank_set_timing.argtypes = [vp, C.c_int]
@@ -61,7 +63,7 @@ def _load():
     lib.bfly_launch_count.restype = i64
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
                  "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
-                 "bfly_search_host", "bfly_debug_fft_tc"):
+                 "bfly_search_host", "bfly_debug_fft_tc", "bfly_tails", "bfly_hits_map"):
         getattr(lib, name).restype = C.c_int
     return lib, path
 
@@ -206,6 +208,52 @@ def butterfly_map(bank: Bank, rho_max: torch.Tensor, arg_lag: torch.Tensor, kapp
                                         n_fbins * n_tbins),
                                    _dev(counters, torch.int64, "counters", bank.device, 2),
                                    _stream(bank.device)), "bfly_butterfly_map")
+    return map_out, counters
+
+
+def tails(bank: Bank, x: torch.Tensor, kappa: float, capacity: int, lag_begin: int = 0,
+          lag_end: int | None = None, n_hits: torch.Tensor | None = None):
+    """bfly_tails on torch's current stream.  Returns (sigma fp32[T], hit_template int32[capacity],
+    hit_lag int32[capacity], hit_rho fp32[capacity], n_hits int64[1]); the hit arrays are in no
+    particular order and valid up to min(n_hits, capacity).  n_hits is incremented (created
+    zeroed if None)."""
+    T = len(bank)
+    n = x.numel()
+    lag_end = n - bank.L + 1 if lag_end is None else lag_end
+    dev = torch.device("cuda", bank.device)
+    sigma = torch.empty(T, dtype=torch.float32, device=dev)
+    cap = max(int(capacity), 0)
+    hj = torch.empty(max(cap, 1), dtype=torch.int32, device=dev)
+    hl = torch.empty(max(cap, 1), dtype=torch.int32, device=dev)
+    hr = torch.empty(max(cap, 1), dtype=torch.float32, device=dev)
+    if n_hits is None:
+        n_hits = torch.zeros(1, dtype=torch.int64, device=dev)
+    _check(_lib.bfly_tails(bank._h, _dev(x, torch.float32, "x", bank.device), n, int(lag_begin),
+                           int(lag_end), float(kappa), C.c_void_p(sigma.data_ptr()), cap,
+                           C.c_void_p(hj.data_ptr()), C.c_void_p(hl.data_ptr()),
+                           C.c_void_p(hr.data_ptr()),
+                           _dev(n_hits, torch.int64, "n_hits", bank.device, 1),
+                           _stream(bank.device)), "bfly_tails")
+    return sigma, hj, hl, hr, n_hits
+
+
+def hits_map(bank: Bank, hit_template: torch.Tensor, hit_lag: torch.Tensor, n_hits: int,
+             lag_origin: int, samples_per_tbin: int, f_lo_hz: float, df_hz: float, n_fbins: int,
+             n_tbins: int, map_out: torch.Tensor | None = None,
+             counters: torch.Tensor | None = None):
+    """bfly_hits_map: one count per hit of a bfly_tails list; accumulates like butterfly_map."""
+    dev = torch.device("cuda", bank.device)
+    if map_out is None:
+        map_out = torch.zeros((n_tbins, n_fbins), dtype=torch.int32, device=dev)
+    if counters is None:
+        counters = torch.zeros(2, dtype=torch.int64, device=dev)
+    _check(_lib.bfly_hits_map(bank._h, _dev(hit_template, torch.int32, "hit_template", bank.device),
+                              _dev(hit_lag, torch.int32, "hit_lag", bank.device), int(n_hits),
+                              int(lag_origin), int(samples_per_tbin), float(f_lo_hz), float(df_hz),
+                              int(n_fbins), int(n_tbins),
+                              _dev(map_out, torch.int32, "map_out", bank.device, n_fbins * n_tbins),
+                              _dev(counters, torch.int64, "counters", bank.device, 2),
+                              _stream(bank.device)), "bfly_hits_map")
     return map_out, counters
 
 

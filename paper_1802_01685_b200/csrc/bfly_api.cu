@@ -112,7 +112,7 @@ void bfly_free_bank(bfly_bank *b)
     cudaFree(b->f0); cudaFree(b->f1); cudaFree(b->phA); cudaFree(b->phB);
     cudaFree(b->inc2); cudaFree(b->ins2); cudaFree(b->rn2); cudaFree(b->xspec);
     cudaFree(b->xh); cudaFree(b->rn2p); cudaFree(b->qs);
-    cudaFree(b->ys); cudaFree(b->rn2s); cudaFree(b->maxbits);
+    cudaFree(b->ys); cudaFree(b->rn2s); cudaFree(b->maxbits); cudaFree(b->racf); cudaFree(b->wspec);
     cudaFree(b->packed); cudaFree(b->x_stage); cudaFree(b->rho_stage); cudaFree(b->arg_stage);
     cudaFree(b->map_stage); cudaFree(b->cnt_stage);
     if (b->ev_start) cudaEventDestroy(b->ev_start);
@@ -272,6 +272,56 @@ int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int
     if (form == BFLY_FORM_FFT)
         return launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
     return launch_fft_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+}
+
+int bfly_tails(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int64_t lag_begin,
+               int64_t lag_end, float kappa, float *sigma_dev, int64_t capacity,
+               int32_t *hit_template_dev, int32_t *hit_lag_dev, float *hit_rho_dev,
+               uint64_t *n_hits_dev, void *stream)
+{
+    if (!bank || !x_dev || !sigma_dev || !n_hits_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (capacity < 0 || (capacity > 0 && (!hit_template_dev || !hit_lag_dev || !hit_rho_dev))) {
+        set_error("hit list arrays missing for capacity %lld", (long long)capacity);
+        return BFLY_EINVAL;
+    }
+    if (!std::isfinite(kappa) || !(kappa > 0.0f)) { set_error("kappa must be finite and > 0"); return BFLY_EINVAL; }
+    if (n_samples < bank->L) { set_error("n_samples < L"); return BFLY_EINVAL; }
+    if (n_samples >= (1LL << 31)) { set_error("segment too long (n_samples must be < 2^31)"); return BFLY_ERANGE; }
+    if (lag_begin < 0 || lag_end < lag_begin || lag_end > n_samples - bank->L + 1) {
+        set_error("lag range [%lld, %lld) outside the valid lags [0, %lld)", (long long)lag_begin,
+                  (long long)lag_end, (long long)(n_samples - bank->L + 1));
+        return BFLY_EINVAL;
+    }
+    if (bank->L < BFLY_TC_MIN_L) {
+        set_error("bfly_tails needs L >= %d (L = %d)", BFLY_TC_MIN_L, bank->L);
+        return BFLY_EUNSUPPORTED;
+    }
+    bfly_bank *b = const_cast<bfly_bank *>(bank);
+    BFLY_CUDA(cudaSetDevice(b->device));
+    int rc = reserve_for(b, n_samples);
+    if (rc) return rc;
+    if (!b->racf) BFLY_CUDA(cudaMalloc((void **)&b->racf, sizeof(double) * FFT_MAX_L));
+    if (!b->wspec) BFLY_CUDA(cudaMalloc((void **)&b->wspec, sizeof(float) * FFT_B));
+    cudaStream_t st = (cudaStream_t)stream;
+    // rn2 serves the direct tail lags of the kernel's geometry in the other mode; not needed here
+    return launch_tails_tc(b, x_dev, n_samples, lag_begin, lag_end, kappa, sigma_dev, capacity,
+                           hit_template_dev, hit_lag_dev, hit_rho_dev,
+                           (unsigned long long *)n_hits_dev, st);
+}
+
+int bfly_hits_map(const bfly_bank *bank, const int32_t *hit_template_dev, const int32_t *hit_lag_dev,
+                  int64_t n_hits, int64_t lag_origin, int32_t samples_per_tbin, double f_lo_hz,
+                  double df_hz, int32_t n_fbins, int32_t n_tbins, uint32_t *map_dev,
+                  uint64_t *counters_dev, void *stream)
+{
+    if (!bank || !map_dev || !counters_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n_hits < 0 || (n_hits > 0 && (!hit_template_dev || !hit_lag_dev))) { set_error("bad hit list"); return BFLY_EINVAL; }
+    if (!(df_hz > 0.0) || !std::isfinite(df_hz) || !std::isfinite(f_lo_hz)) { set_error("df must be finite and > 0, f_lo finite"); return BFLY_EINVAL; }
+    if (samples_per_tbin <= 0 || n_fbins <= 0 || n_tbins <= 0 || lag_origin < 0) { set_error("bad map geometry"); return BFLY_EINVAL; }
+    BFLY_CUDA(cudaSetDevice(bank->device));
+    return launch_hits_map(bank, hit_template_dev, hit_lag_dev, n_hits, lag_origin, samples_per_tbin,
+                           f_lo_hz, df_hz, n_fbins, n_tbins, map_dev, (unsigned long long *)counters_dev,
+                           (cudaStream_t)stream);
 }
 
 int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream)

@@ -143,4 +143,49 @@ int launch_map(const bfly_bank *b, const float *rho_max, const int32_t *arg_lag,
     return BFLY_OK;
 }
 
+// The map of a hit list (bfly_tails): one count per hit at (time bin of the hit's lag, frequency
+// bin of its template's f0) -- the same coordinates as map_kernel (reading C10), but a template
+// may contribute many hits per segment: the paper's trajectory map.
+__global__ void __launch_bounds__(256) hits_map_kernel(int64_t n_hits, int64_t T, const double *__restrict__ f0,
+                                                       const int32_t *__restrict__ hit_template,
+                                                       const int32_t *__restrict__ hit_lag,
+                                                       int64_t lag_origin, int32_t samples_per_tbin,
+                                                       double f_lo, double df, int32_t n_fbins,
+                                                       int32_t n_tbins, uint32_t *__restrict__ map,
+                                                       unsigned long long *__restrict__ counters)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool hit = false, dropped = false;
+    if (i < n_hits) {
+        hit = true;
+        const int64_t j = hit_template[i];
+        const int64_t tbin = (lag_origin + (int64_t)hit_lag[i]) / samples_per_tbin;
+        const double fb = (j >= 0 && j < T) ? floor((f0[j] - f_lo) / df) : -1.0;
+        if (tbin >= 0 && tbin < n_tbins && fb >= 0.0 && fb < (double)n_fbins)
+            atomicAdd(&map[tbin * (int64_t)n_fbins + (int64_t)fb], 1u);
+        else
+            dropped = true;
+    }
+    const unsigned mh = __ballot_sync(0xffffffffu, hit);
+    const unsigned md = __ballot_sync(0xffffffffu, dropped);
+    if ((threadIdx.x & 31) == 0) {
+        if (mh) atomicAdd(&counters[0], (unsigned long long)__popc(mh));
+        if (md) atomicAdd(&counters[1], (unsigned long long)__popc(md));
+    }
+}
+
+int launch_hits_map(const bfly_bank *b, const int32_t *hit_template, const int32_t *hit_lag,
+                    int64_t n_hits, int64_t lag_origin, int32_t samples_per_tbin, double f_lo,
+                    double df, int32_t n_fbins, int32_t n_tbins, uint32_t *map,
+                    unsigned long long *counters, cudaStream_t stream)
+{
+    if (n_hits == 0) return BFLY_OK;
+    hits_map_kernel<<<(unsigned)((n_hits + 255) / 256), 256, 0, stream>>>(
+        n_hits, b->T, b->f0, hit_template, hit_lag, lag_origin, samples_per_tbin, f_lo, df, n_fbins,
+        n_tbins, map, counters);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    return BFLY_OK;
+}
+
 }  // namespace bfly

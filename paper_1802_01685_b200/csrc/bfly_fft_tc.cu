@@ -89,7 +89,7 @@ tc_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_be
 // -inf past the last lag so that such a slot never wins the maximum).  float64 sums as in A2.
 __global__ void __launch_bounds__(256)
 tc_norm_kernel(const float *__restrict__ x, int32_t L, int64_t lag_begin, int64_t n_fft_lags,
-               const double *__restrict__ qs, float *__restrict__ rn2p, int64_t n_slots)
+               const double *__restrict__ qs, float *__restrict__ rn2p, int64_t n_slots, int tails)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= n_slots) return;
@@ -98,6 +98,10 @@ tc_norm_kernel(const float *__restrict__ x, int32_t L, int64_t lag_begin, int64_
     const int w = tid >> 5, g = (tid >> 2) & 7, t = tid & 3;
     const int n = (4 * w + (slot >> 1)) + 64 * (2 * t + (slot & 1)) + 512 * g;
     const int64_t i = b * TCV + n;
+    if (tails) {       // kappa-sigma tails: the block's scale alone, 0 past the last lag (never a hit)
+        rn2p[idx] = i < n_fft_lags ? (float)qs[b] : 0.0f;
+        return;
+    }
     if (i >= n_fft_lags) { rn2p[idx] = -INFINITY; return; }
     const float *p = x + lag_begin + i;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
@@ -110,6 +114,62 @@ tc_norm_kernel(const float *__restrict__ x, int32_t L, int64_t lag_begin, int64_
     for (; k < L; ++k) { const double v = (double)__ldg(p + k); a0 = fma(v, v, a0); }
     const double n2 = (a0 + a1) + (a2 + a3);
     rn2p[idx] = n2 > 0.0 ? (float)(qs[b] / n2) : 0.0f;
+}
+
+// ------------------------------------------------------------------------------------------
+// The predictor step of the kappa-sigma tails (sigma "computed in a predictor step by
+// Parseval's Theorem"; readings S1-S3 of DESIGN.md).  With R[d] the circular autocorrelation of
+// the N-sample segment, sum_tau |z~(tau)|^2 of the circular correlation z~ of the segment with a
+// template g of L <= B/2 samples is sum_d R[d] A_g[d] = (1/B) sum_m |G[m]|^2 W[m], where A_g is the
+// template's autocorrelation, G its length-B spectrum (the one the correlate kernel computes
+// anyway) and W the length-B transform of R restricted to |d| < L: one dot product per template.
+__global__ void __launch_bounds__(256)
+tc_autocorr_kernel(const float *__restrict__ x, int64_t n_samples, double *__restrict__ racf)
+{
+    __shared__ double part[8];
+    const int64_t d = blockIdx.x;
+    double a = 0.0;
+    for (int64_t n = threadIdx.x; n < n_samples; n += 256) {
+        int64_t m = n + d;
+        if (m >= n_samples) m -= n_samples;
+        a = fma((double)__ldg(x + n), (double)__ldg(x + m), a);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += part[w];
+        racf[d] = t;
+    }
+}
+
+// W[m] = sum_{|d| < L} R[|d|] exp(2 pi i m d / B) (real), written where the correlate kernel's
+// threads find it next to G: float index word + half of operand_slot(m).
+__global__ void __launch_bounds__(fft32::NT, 1)
+tc_wspec_kernel(const double *__restrict__ racf, int32_t L, float *__restrict__ wspec)
+{
+    extern __shared__ float2 smem[];
+    const fft32::Smem sm = fft32::carve(smem);
+    const int t = threadIdx.x;
+    fft32::fill_tables(sm, t);
+    float2 v[fft32::PTS];
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) {
+        const int d = t + fft32::NT * s;
+        float r = 0.0f;
+        if (d < L) r = (float)racf[d];
+        else if (FFT_B - d < L) r = (float)racf[FFT_B - d];
+        v[s] = make_float2(r, 0.0f);
+    }
+    fft32::fft8192(v, sm, t);
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) {
+        int word, half;
+        operand_slot(t + fft32::NT * s, word, half);
+        wspec[word + half] = v[s].x;
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -207,13 +267,29 @@ __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t b
 // "full(b)", so every warp has finished passes A, B of block b and hence passes C, D of block
 // b - 2, the previous user of that buffer.  X_b is staged by one 32 KB cp.async.bulk per block,
 // two blocks ahead, into two slots (the sequence of blocks simply continues across templates).
+// TAILS = true is the paper's own reduction instead of max / argmax (bfly_tails; readings S1-S3):
+// per template sigma by the Parseval predictor above, then every valid lag whose magnitude
+// exceeds kappa sigma is appended to a hit list (one atomic per hit; hits are rare by design).
+struct TailArgs {
+    const float4 *wspec;       // W in the operand layout (tc_wspec_kernel)
+    double sig_norm;           // 1 / (2 N B): sum_m |G|^2 W -> sigma^2 ||cos phi||^2 (gs holds G itself)
+    float kappa;
+    float *sigma;              // [T]
+    long long capacity;
+    int32_t *hit_template, *hit_lag;
+    float *hit_rho;
+    unsigned long long *n_hits;
+};
+
+template <bool TAILS>
 __global__ void __launch_bounds__(NT, 1)
 tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const uint64_t *__restrict__ phB, const float *__restrict__ inc2,
                     const float *__restrict__ ins2, const uint4 *__restrict__ xh,
                     const float4 *__restrict__ rn2p, const float *__restrict__ x,
                     const float *__restrict__ rn2, int64_t lag_begin, int32_t n_blocks,
-                    int32_t n_tail, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
+                    int32_t n_tail, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag,
+                    const TailArgs ta)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const TcSmem sm = carve_tc(smem_raw);
@@ -346,6 +422,35 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             }
         }
         __syncthreads();
+        float thr = 0.0f, rsig2 = 0.0f;               // TAILS: kappa^2 sigma^2 / inc2 and inc2 / sigma^2
+        if (TAILS) {
+            float acc = 0.0f;
+#pragma unroll
+            for (int ci = 0; ci < 4; ++ci) {
+                const uint4 gq = sm.gs[ci * NT + tid];
+                const float4 wv = __ldg(ta.wspec + ci * NT + tid);
+                const float2 r0 = __half22float2(as_h2(gq.x)), i0 = __half22float2(as_h2(gq.y));
+                const float2 r1 = __half22float2(as_h2(gq.z)), i1 = __half22float2(as_h2(gq.w));
+                acc = fmaf(fmaf(r0.x, r0.x, i0.x * i0.x), wv.x, acc);
+                acc = fmaf(fmaf(r0.y, r0.y, i0.y * i0.y), wv.y, acc);
+                acc = fmaf(fmaf(r1.x, r1.x, i1.x * i1.x), wv.z, acc);
+                acc = fmaf(fmaf(r1.y, r1.y, i1.y * i1.y), wv.w, acc);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            float *part = reinterpret_cast<float *>(sm.red);
+            if (lane == 0) part[w] = acc;
+            __syncthreads();
+            double tot = 0.0;
+#pragma unroll
+            for (int ww = 0; ww < 16; ++ww) tot += (double)part[ww];      // same order in every thread
+            const float s2c = (float)(tot * ta.sig_norm);                 // sigma^2 ||cos phi||^2 (>= 0 up to rounding)
+            const float sig2 = fmaxf(s2c * ic, 0.0f);
+            if (tid == 0) ta.sigma[j] = sqrtf(sig2);
+            thr = ta.kappa * ta.kappa * fmaxf(s2c, 0.0f);
+            rsig2 = sig2 > 0.0f ? ic / sig2 : 0.0f;
+            if (!(thr > 0.0f)) thr = INFINITY;                           // sigma = 0: no hits (S3)
+        }
 
         // ---- A4: passes A, B of one block: Y = X_b . G in packed fp16, straight into the
         //      fragments of pass A; result to exchange buffer wb; one arrival per warp
@@ -401,8 +506,23 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 cpair z, zu;
                 chain2<false, TC_HALF>(k, rbuf, 4 * w + i, lane, z, zu, nowu);
                 const float2 q = __fmul2_rn(__ffma2_rn(z.i, z.i, __fmul2_rn(z.r, z.r)), rr[i]);
-                if (q.x > best) { best = q.x; code = 8 * b + 2 * i; }
-                if (q.y > best) { best = q.y; code = 8 * b + 2 * i + 1; }
+                if (TAILS) {
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const float qe = e ? q.y : q.x;
+                        if (qe > thr) {
+                            const unsigned long long at = atomicAdd(ta.n_hits, 1ull);
+                            if (at < (unsigned long long)ta.capacity) {
+                                ta.hit_template[at] = (int32_t)j;
+                                ta.hit_lag[at] = (int32_t)(lag_begin + (int64_t)b * TCV + (4 * w + i) + 64 * (2 * t + e) + 512 * g);
+                                ta.hit_rho[at] = sqrtf(qe * rsig2);
+                            }
+                        }
+                    }
+                } else {
+                    if (q.x > best) { best = q.x; code = 8 * b + 2 * i; }
+                    if (q.y > best) { best = q.y; code = 8 * b + 2 * i + 1; }
+                }
             }
         }
         // ---- tail lags (direct sums) and the CTA-wide maximum, ties to the smallest lag
@@ -412,8 +532,24 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 c += sm.tail[(ww * MAX_TAIL + tid) * 2];
                 s += sm.tail[(ww * MAX_TAIL + tid) * 2 + 1];
             }
-            const float q = fmaf(s, s, c * c) * __ldg(rn2 + (int64_t)n_blocks * TCV + tid);
-            if (q > best) { best = q; code = 8 * n_blocks + tid; }
+            if (TAILS) {
+                const float q = fmaf(s, s, c * c);                       // raw samples: no block scale
+                if (q > thr) {
+                    const unsigned long long at = atomicAdd(ta.n_hits, 1ull);
+                    if (at < (unsigned long long)ta.capacity) {
+                        ta.hit_template[at] = (int32_t)j;
+                        ta.hit_lag[at] = (int32_t)(lag_begin + (int64_t)n_blocks * TCV + tid);
+                        ta.hit_rho[at] = sqrtf(q * rsig2);
+                    }
+                }
+            } else {
+                const float q = fmaf(s, s, c * c) * __ldg(rn2 + (int64_t)n_blocks * TCV + tid);
+                if (q > best) { best = q; code = 8 * n_blocks + tid; }
+            }
+        }
+        if (TAILS) {
+            __syncthreads();                            // red[], tail[], gs, exch are reused by the next template
+            continue;
         }
         unsigned long long p = 0ull;
         if (best > 0.0f) {
@@ -500,13 +636,16 @@ int64_t tc_blocks_needed(int64_t n_lags)
     return nb;
 }
 
-int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
-                  int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream)
+static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                            int64_t lag_end, float *rho_max, int32_t *arg_lag, const TailArgs *tails,
+                            cudaStream_t stream)
 {
     static bool attr_set = false;
     if (!attr_set) {
         BFLY_CUDA(cudaFuncSetAttribute(tc_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_wspec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         attr_set = true;
     }
     const int64_t n_lags = lag_end - lag_begin;
@@ -524,20 +663,64 @@ int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t
         BFLY_CUDA(cudaGetLastError());
         const int64_t n_slots = n_blocks * TCV;
         tc_norm_kernel<<<(unsigned)((n_slots + 255) / 256), 256, 0, stream>>>(
-            x, b->L, lag_begin, n_lags - n_tail, b->qs, b->rn2p, n_slots);
+            x, b->L, lag_begin, n_lags - n_tail, b->qs, b->rn2p, n_slots, tails ? 1 : 0);
         count_launch();
         BFLY_CUDA(cudaGetLastError());
     }
     const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
     core_timer_start(b, stream);
-    tc_correlate_kernel<<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
-        b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
-        reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
-        rho_max, arg_lag);
+    if (tails)
+        tc_correlate_kernel<true><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
+            b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
+            reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
+            rho_max, arg_lag, *tails);
+    else
+        tc_correlate_kernel<false><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
+            b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
+            reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
+            rho_max, arg_lag, TailArgs{});
     core_timer_stop(b, stream);
     count_launch();
     BFLY_CUDA(cudaGetLastError());
     return BFLY_OK;
+}
+
+int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                  int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream)
+{
+    return launch_tc_common(b, x, n_samples, lag_begin, lag_end, rho_max, arg_lag, nullptr, stream);
+}
+
+// bfly_tails: predictor step (autocorrelation of the segment, its transform W), then the
+// correlate kernel in TAILS mode.  racf / wspec are workspace of the bank (sized by the caller).
+int launch_tails_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                    int64_t lag_end, float kappa, float *sigma, int64_t capacity,
+                    int32_t *hit_template, int32_t *hit_lag, float *hit_rho,
+                    unsigned long long *n_hits, cudaStream_t stream)
+{
+    tc_autocorr_kernel<<<(unsigned)b->L, 256, 0, stream>>>(x, n_samples, b->racf);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    // the attribute for tc_wspec_kernel is set in launch_tc_common; make sure it ran once
+    static bool attr_set = false;
+    if (!attr_set) {
+        BFLY_CUDA(cudaFuncSetAttribute(tc_wspec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
+        attr_set = true;
+    }
+    tc_wspec_kernel<<<1, fft32::NT, fft32::FFT_SMEM, stream>>>(b->racf, b->L, b->wspec);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    TailArgs ta;
+    ta.wspec = reinterpret_cast<const float4 *>(b->wspec);
+    ta.sig_norm = 1.0 / (2.0 * (double)n_samples * (double)FFT_B);
+    ta.kappa = kappa;
+    ta.sigma = sigma;
+    ta.capacity = (long long)capacity;
+    ta.hit_template = hit_template;
+    ta.hit_lag = hit_lag;
+    ta.hit_rho = hit_rho;
+    ta.n_hits = n_hits;
+    return launch_tc_common(b, x, n_samples, lag_begin, lag_end, nullptr, nullptr, &ta, stream);
 }
 
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream)

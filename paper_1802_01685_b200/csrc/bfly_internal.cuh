@@ -31,6 +31,8 @@ struct bfly_bank {
     int64_t rn2p_cap;         // floats (4096 per block)
     double *qs;               // BFLY_FORM_FFT_TC: per-block scale 2^(-2s) / S16^2
     int64_t qs_cap;
+    double *racf;             // bfly_tails: circular autocorrelation of the segment, lags 0..L-1
+    float *wspec;             // bfly_tails: its length-8192 transform W in the operand layout
     __half *ys;               // BFLY_FORM_DENSE_TC: eight shifted fp16 copies of the scaled series
     int64_t ys_cap;
     float *rn2s;              // BFLY_FORM_DENSE_TC: 1 / (n2 scale^2), padded to whole lag tiles
@@ -97,6 +99,14 @@ int64_t fft_blocks_needed(int32_t L, int64_t n_lags);
 int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                   int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int64_t tc_blocks_needed(int64_t n_lags);
+int launch_tails_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                    int64_t lag_end, float kappa, float *sigma, int64_t capacity,
+                    int32_t *hit_template, int32_t *hit_lag, float *hit_rho,
+                    unsigned long long *n_hits, cudaStream_t stream);
+int launch_hits_map(const bfly_bank *b, const int32_t *hit_template, const int32_t *hit_lag,
+                    int64_t n_hits, int64_t lag_origin, int32_t samples_per_tbin, double f_lo,
+                    double df, int32_t n_fbins, int32_t n_tbins, uint32_t *map,
+                    unsigned long long *counters, cudaStream_t stream);
 int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin, int64_t lag_end,
                     float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream);

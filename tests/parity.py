@@ -78,3 +78,53 @@ def check_map(f0, rho_gpu, arg_gpu, map_gpu, counters_gpu, rho_o, arg_o, exempt,
     l1 = np.abs(m_full.astype(np.int64) - m_self.astype(np.int64)).sum()
     assert l1 <= 2 * int(amb.sum()), f"R3(iii): L1 {l1} > 2 x {int(amb.sum())} ambiguous"
     return int(amb.sum())
+
+
+SIGMA_RTOL = 1e-3    # R5: relative tolerance on sigma_j
+
+
+def check_tails(x, fs, L, f0, f1, kappa, sigma_gpu, hit_j, hit_lag, hit_rho, total, lag_begin=0,
+                lag_end=None):
+    """R5: the kappa-sigma tails of the CUDA path against oracle.sigma / the oracle's
+    series.  rho_sigma = rho ||x_tau|| / sigma, so north_star's |d rho| <= 2e-4 becomes the
+    per-hit tolerance tol = 2e-4 ||x_tau|| / sigma_j + SIGMA_RTOL rho_sigma.  (i) sigma within
+    SIGMA_RTOL; (ii) every GPU hit is a hit of the oracle up to tol, with its value within tol;
+    (iii) every oracle hit above kappa + tol is in the GPU list; (iv) no duplicates, and the
+    total equals the list length when nothing overflowed."""
+    f0 = np.asarray(f0, np.float64)
+    f1 = np.asarray(f1, np.float64)
+    lag_end = len(x) - L + 1 if lag_end is None else lag_end
+    sig_o = np.array([oracle.sigma(x, fs, L, a, b) for a, b in zip(f0, f1)])
+    sigma_gpu = np.asarray(sigma_gpu, np.float64)
+    ok = sig_o > 0
+    assert np.all(sigma_gpu[~ok] == 0.0)
+    assert np.abs(sigma_gpu[ok] / sig_o[ok] - 1.0).max(initial=0.0) <= SIGMA_RTOL, \
+        f"R5(i): sigma off by {np.abs(sigma_gpu[ok] / sig_o[ok] - 1.0).max():.2e}"
+    n2 = oracle.sliding_n2(x, L, lag_begin, lag_end)
+    got = {}
+    for j, lag, r in zip(np.asarray(hit_j), np.asarray(hit_lag), np.asarray(hit_rho, np.float64)):
+        assert (int(j), int(lag)) not in got, "R5(iv): duplicate hit"
+        assert lag_begin <= lag < lag_end
+        got[(int(j), int(lag))] = r
+    assert total >= len(got)
+    n_oracle = n_border = 0
+    for j in range(len(f0)):
+        if not ok[j]:
+            continue
+        rs = oracle.rho_series(x, fs, L, f0[j], f1[j], lag_begin, lag_end) * np.sqrt(n2) / sig_o[j]
+        tol = 2e-4 * np.sqrt(n2) / sig_o[j] + SIGMA_RTOL * rs
+        mine = {lag for (jj, lag) in got if jj == j}
+        for lag in mine:
+            i = lag - lag_begin
+            assert rs[i] > kappa - tol[i], f"R5(ii): gpu hit ({j}, {lag}) has oracle rho_sigma {rs[i]}"
+            assert abs(got[(j, lag)] - rs[i]) <= tol[i], \
+                f"R5(ii): value at ({j}, {lag}): gpu {got[(j, lag)]} oracle {rs[i]} tol {tol[i]}"
+        sure = np.nonzero(rs > kappa + tol)[0]
+        n_oracle += int((rs > kappa).sum())
+        n_border += int(((rs > kappa - tol) & (rs <= kappa + tol)).sum())
+        if total == len(got):                       # nothing overflowed: the list is complete
+            missing = [lag_begin + int(i) for i in sure if lag_begin + int(i) not in mine]
+            assert not missing, f"R5(iii): template {j} misses sure hits at lags {missing[:5]}"
+    if total == len(got):
+        assert abs(total - n_oracle) <= n_border
+    return n_oracle, n_border

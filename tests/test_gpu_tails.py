@@ -1,0 +1,97 @@
+"""GPU parity of the kappa-sigma tails (bfly_tails, bfly_hits_map; SURVEY 8(f) rank 2,
+PAPER.md:70, 120) against the float64 oracle: rule R5 of DESIGN.md.  Needs a B200."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import bank_grid, default_map_grid, get_config, make_data, sub_bank_indices
+
+from parity import check_tails
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def bfly():
+    import paper_1802_01685_b200 as b
+    return b
+
+
+def _tails(bfly, fs, L, f0, f1, x, kappa, capacity, lb=0, le=None):
+    bank = bfly.make_bank(fs, L, f0, f1)
+    xd = torch.from_numpy(x).cuda()
+    sig, hj, hl, hr, n = bfly.tails(bank, xd, kappa, capacity, lb, le)
+    torch.cuda.synchronize()
+    total = int(n.item())
+    k = min(total, capacity)
+    return bank, sig.cpu().numpy(), hj.cpu().numpy()[:k], hl.cpu().numpy()[:k], hr.cpu().numpy()[:k], total, (hj, hl)
+
+
+def test_tails_small_segment_with_injection(bfly):
+    rng = np.random.default_rng(21)
+    fs, L, N = 2048.0, 2048, 12000
+    x = rng.standard_normal(N)
+    f0 = np.concatenate([[600.0], rng.uniform(100, 900, 39)])
+    f1 = np.concatenate([[-200.0], rng.uniform(-300, 300, 39)])
+    hc, _ = oracle.template(fs, L, 600.0, -200.0)
+    x[3000:3000 + L] += 0.25 * hc
+    x = x.astype(np.float32)
+    kappa = 3.6
+    bank, sig, hj, hl, hr, total, dev = _tails(bfly, fs, L, f0, f1, x, kappa, 1 << 16)
+    n_oracle, n_border = check_tails(x, fs, L, f0, f1, kappa, sig, hj, hl, hr, total)
+    assert n_oracle > 50 and 3000 in hl[hj == 0]
+    # the map of the hit list = the histogram of the list (integer, exact)
+    grid = dict(samples_per_tbin=128, f_lo_hz=0.0, df_hz=1.0, n_fbins=1001, n_tbins=(N + 127) // 128)
+    m, c = bfly.hits_map(bank, dev[0], dev[1], total, 77, **grid)
+    want = np.zeros((grid["n_tbins"], grid["n_fbins"]), np.uint32)
+    dropped = 0
+    for j, lag in zip(hj, hl):
+        tb, fb = (77 + int(lag)) // 128, int(np.floor(f0[j]))
+        if tb < grid["n_tbins"] and 0 <= fb < grid["n_fbins"]:
+            want[tb, fb] += 1
+        else:
+            dropped += 1
+    np.testing.assert_array_equal(m.cpu().numpy().view(np.uint32), want)
+    assert c.cpu().numpy().tolist() == [total, dropped]
+    # determinism of the SET of hits, and the overflow rule: the count still counts everything
+    _, sig2, hj2, hl2, hr2, total2, _ = _tails(bfly, fs, L, f0, f1, x, kappa, 1 << 16)
+    assert total2 == total and np.array_equal(sig2, sig)
+    assert sorted(zip(hj2.tolist(), hl2.tolist(), hr2.tolist())) == sorted(zip(hj.tolist(), hl.tolist(), hr.tolist()))
+    _, _, hj3, hl3, _, total3, _ = _tails(bfly, fs, L, f0, f1, x, kappa, 10)
+    assert total3 == total and len(hj3) == 10
+    assert set(zip(hj3.tolist(), hl3.tolist())) <= set(zip(hj.tolist(), hl.tolist()))
+
+
+@pytest.mark.parametrize("index,n_random,kappa", [(4, 24, 4.0), (3, 16, 3.8), (2, 12, 4.2)])
+def test_tails_sub_bank_of_config(bfly, index, n_random, kappa):
+    cfg = get_config(index)
+    n = 65536 if index == 2 else None                # one 16-s segment of the 32-s series
+    x = make_data(cfg, n)
+    f0a, f1a = bank_grid(cfg)
+    idx = sub_bank_indices(cfg, n_random, max_track=8)
+    f0, f1 = f0a[idx], f1a[idx]
+    bank, sig, hj, hl, hr, total, _ = _tails(bfly, cfg.fs_hz, cfg.L, f0, f1, x, kappa, 1 << 18)
+    n_oracle, _ = check_tails(x, cfg.fs_hz, cfg.L, f0, f1, kappa, sig, hj, hl, hr, total)
+    assert n_oracle > 0
+
+
+def test_tails_lag_subrange_scale_and_edges(bfly):
+    rng = np.random.default_rng(23)
+    fs, L, N = 1024.0, 512, 20000
+    x = rng.standard_normal(N).astype(np.float32)
+    f0, f1 = rng.uniform(50, 450, 9), rng.uniform(-150, 150, 9)
+    for lb, le in ((0, N - L + 1), (1234, 9000), (17, 17 + 4096), (17, 17 + 4097), (500, 501)):
+        _, sig, hj, hl, hr, total, _ = _tails(bfly, fs, L, f0, f1, x, 3.5, 1 << 16, lb, le)
+        check_tails(x, fs, L, f0, f1, 3.5, sig, hj, hl, hr, total, lb, le)
+    xs = (x * np.float32(4096.0)).astype(np.float32)          # rho_sigma is scale invariant
+    _, sig_s, hj_s, hl_s, hr_s, total_s, _ = _tails(bfly, fs, L, f0, f1, xs, 3.5, 1 << 16)
+    check_tails(xs, fs, L, f0, f1, 3.5, sig_s, hj_s, hl_s, hr_s, total_s)
+    z = np.zeros(N, np.float32)                               # S3: sigma = 0, no hits
+    _, sig0, hj0, _, _, total0, _ = _tails(bfly, fs, L, f0, f1, z, 3.5, 16)
+    assert total0 == 0 and np.all(sig0 == 0.0)
+    with pytest.raises(bfly.BflyError):                       # needs L >= BFLY_TC_MIN_L
+        _tails(bfly, 512.0, 64, [50.0], [1.0], x, 3.5, 16)
+    with pytest.raises(bfly.BflyError):                       # kappa must be > 0
+        _tails(bfly, fs, L, f0, f1, x, 0.0, 16)
