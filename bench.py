@@ -328,6 +328,21 @@ def main():
                                                "peak_basis": bf16_basis},
                                   "note": "same rows A3-A7 as a Hankel x template contraction on tcgen05; "
                                           "109x the flops of the FFT form, hence not the default"}}
+            # the paper's own reduction on the same kernel: sigma by Parseval + all tails above
+            # kappa sigma (bfly_tails), whole bank, kappa = 5.5 (about 1e5 hits in noise)
+            bank.set_timing(True)
+            tms, nh = [], 0
+            for i in range(2):
+                sg, hj, hl, hr, nhits = bfly.tails(bank, xd, 5.5, 1 << 22)
+                if i:
+                    tms.append(bank.core_ms())
+                nh = int(nhits.item())
+            tsec = float(np.mean(tms)) * 1e-3
+            other["tails"] = {"kernel": "tc_correlate_kernel<TAILS>", "templates": T, "kappa_sigma": 5.5,
+                              "kernel_ms": tsec * 1e3, "value": corr_step / tsec, "unit": UNIT, "hits": nh,
+                              "note": "PAPER.md:70, 120: sigma per template by the Parseval predictor, "
+                                      "every lag with rho > kappa sigma appended to a hit list"}
+            bank.set_timing(False)
         # ---- the oracle beside it, on this box's host cores, on a bounded sample
         idx = sub_bank_indices(cfg, 8192, seed=7, halfwidth=0, max_track=0)
         cv, cn, cs, cores = time_oracle(cfg, x, f0a[idx], f1a[idx], args.cpu_seconds)

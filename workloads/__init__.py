@@ -12,7 +12,7 @@ PAPER.md:64, 68, 124) are not available; these inputs stand in for them.
 """
 from .configs import CONFIGS, Config, get_config
 from .generators import (bank_grid, make_data, sub_bank_indices,
-                         default_map_grid)
+                         default_map_grid, permutation)
 
 __all__ = ["CONFIGS", "Config", "get_config", "bank_grid", "make_data",
-           "sub_bank_indices", "default_map_grid"]
+           "sub_bank_indices", "default_map_grid", "permutation"]

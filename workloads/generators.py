@@ -131,3 +131,10 @@ def sub_bank_indices(cfg: Config, n_random: int, seed: int = 0,
         lo, hi = edges[:-1], np.maximum(edges[1:], edges[:-1] + 1)
         idx.update(int(i) for i in np.minimum(rng.integers(lo, hi), T - 1))
     return np.array(sorted(idx), dtype=np.int64)
+
+
+def permutation(n: int, seed: int) -> np.ndarray:
+    """Seeded uniformly random permutation of range(n) (int32): the input of the time-randomised
+    control (reading T1).  Input generation only: both the oracle and the CUDA path
+    receive this array."""
+    return np.random.default_rng(seed).permutation(n).astype(np.int32)
