@@ -171,6 +171,34 @@ int bfly_hits_map(const bfly_bank *bank, const int32_t *hit_template_dev, const 
                   double df_hz, int32_t n_fbins, int32_t n_tbins, uint32_t *map_dev,
                   uint64_t *counters_dev, void *stream);
 
+/* ---- Reading the output of two series: control, coincidence, pseudo-spectra ----------------
+ * PAPER.md:68 (control "following time-randomisation of the H1 and L1 data ... maximal entropy,
+ * keeping histograms the same"), PAPER.md:124 ("pseudo-spectra of simultaneous rho > kappa sigma
+ * in H1 and L1 ... by independent counts and by simultaneous counts with frequency pairs within
+ * Delta f = 50 Hz").  Readings T1-T3 of DESIGN.md.  These three calls need no bank; they run on
+ * the CURRENT device, asynchronously on `stream`; all pointers are DEVICE, caller-owned.
+ *
+ * T1  out_dev[i] = x_dev[perm_dev[i]], i < n.  perm_dev (int32) is an INPUT: a permutation of
+ *     0..n-1 drawn by the caller's seeded generator (the library draws no random numbers).  An
+ *     index outside [0, n) writes 0 and sets *bad_dev (int32, may be NULL) to 1.  out_dev must
+ *     not alias x_dev.  The control is then the same bfly_correlate / bfly_tails on out_dev. */
+int bfly_time_randomize(const float *x_dev, const int32_t *perm_dev, int64_t n, float *out_dev,
+                        int32_t *bad_dev, void *stream);
+
+/* T2  Two count maps of the same geometry (uint32 [n_tbins][n_fbins], one count per hit, as
+ *     bfly_butterfly_map / bfly_hits_map write them).  co1_dev[t][f] = map1_dev[t][f] if map2_dev
+ *     has a non-zero bin at the same time bin t within half_width_bins frequency bins of f, else
+ *     0; co2_dev likewise with the roles exchanged.  co1_dev / co2_dev are OVERWRITTEN and must
+ *     not alias the inputs.  n_fbins <= 65536 (BFLY_ERANGE). */
+int bfly_coincidence(const uint32_t *map1_dev, const uint32_t *map2_dev, int32_t n_tbins,
+                     int32_t n_fbins, int32_t half_width_bins, uint32_t *co1_dev,
+                     uint32_t *co2_dev, void *stream);
+
+/* T3  spectrum_dev[f] += sum over t of map_dev[t][f]  (uint64 [n_fbins], ACCUMULATED into, so
+ *     that blocks of a long run add up; the caller zeroes it). */
+int bfly_pseudo_spectrum(const uint32_t *map_dev, int32_t n_tbins, int32_t n_fbins,
+                         uint64_t *spectrum_dev, void *stream);
+
 /* ---- A9 / end-to-end: the whole path on a HOST series ------------------------------------
  * Runs A2-A8 over a HOST series x_host[n_samples] (fp32), cut into chunks of chunk_samples
  * samples with an overlap of L samples (hop = chunk_samples - L): chunk c starts at sample

@@ -18,7 +18,7 @@ from . import build as _build
 __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
            "butterfly_map", "search_host", "launch_count", "lib_path",
            "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC",
-           "debug_fft_tc", "tails", "hits_map"]
+           "debug_fft_tc", "tails", "hits_map", "time_randomize", "coincidence", "pseudo_spectrum"]
 
 FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC, FORM_DENSE_TC = 0, 1, 2, 3, 4
 
@@ -54,6 +54,9 @@ def _load():
     lib.bfly_butterfly_map.argtypes = [vp, vp, vp, f32, i64, i32, f64, f64, i32, i32, vp, vp, vp]
     lib.bfly_tails.argtypes = [vp, vp, i64, i64, i64, f32, vp, i64, vp, vp, vp, vp, vp]
     lib.bfly_hits_map.argtypes = [vp, vp, vp, i64, i64, i32, f64, f64, i32, i32, vp, vp, vp]
+    lib.bfly_time_randomize.argtypes = [vp, vp, i64, vp, vp, vp]
+    lib.bfly_coincidence.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp]
+    lib.bfly_pseudo_spectrum.argtypes = [vp, i32, i32, vp, vp]
     lib.bfly_search_host.argtypes = [vp, vp, i64, i64, f32, i32, f64, f64, i32, i32,
                                      vp, vp, vp, vp, vp]
     lib.bfly_bank_set_timing.argtypes = [vp, C.c_int]
@@ -63,7 +66,8 @@ def _load():
     lib.bfly_launch_count.restype = i64
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
                  "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
-                 "bfly_search_host", "bfly_debug_fft_tc", "bfly_tails", "bfly_hits_map"):
+                 "bfly_search_host", "bfly_debug_fft_tc", "bfly_tails", "bfly_hits_map",
+                 "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum"):
         getattr(lib, name).restype = C.c_int
     return lib, path
 
@@ -255,6 +259,48 @@ def hits_map(bank: Bank, hit_template: torch.Tensor, hit_lag: torch.Tensor, n_hi
                               _dev(counters, torch.int64, "counters", bank.device, 2),
                               _stream(bank.device)), "bfly_hits_map")
     return map_out, counters
+
+
+def time_randomize(x: torch.Tensor, perm: torch.Tensor):
+    """bfly_time_randomize: (x[perm], bad flag int32[1]); perm is an int32 CUDA tensor drawn by the
+    caller's seeded generator."""
+    n = x.numel()
+    dev = x.device.index
+    out = torch.empty_like(x)
+    bad = torch.zeros(1, dtype=torch.int32, device=x.device)
+    with torch.cuda.device(dev):
+        _check(_lib.bfly_time_randomize(_dev(x, torch.float32, "x"), _dev(perm, torch.int32, "perm", dev, n),
+                                        n, C.c_void_p(out.data_ptr()), C.c_void_p(bad.data_ptr()),
+                                        _stream(dev)), "bfly_time_randomize")
+    return out, bad
+
+
+def coincidence(map1: torch.Tensor, map2: torch.Tensor, half_width_bins: int):
+    """bfly_coincidence on two [n_tbins, n_fbins] int32-stored count maps; returns (co1, co2)."""
+    if map1.shape != map2.shape or map1.dim() != 2:
+        raise ValueError("maps must be 2-D and of equal shape")
+    dev = map1.device.index
+    nt, nf = map1.shape
+    c1, c2 = torch.empty_like(map1), torch.empty_like(map2)
+    with torch.cuda.device(dev):
+        _check(_lib.bfly_coincidence(_dev(map1, torch.int32, "map1"), _dev(map2, torch.int32, "map2", dev),
+                                     int(nt), int(nf), int(half_width_bins), C.c_void_p(c1.data_ptr()),
+                                     C.c_void_p(c2.data_ptr()), _stream(dev)), "bfly_coincidence")
+    return c1, c2
+
+
+def pseudo_spectrum(map_: torch.Tensor, spectrum: torch.Tensor | None = None):
+    """bfly_pseudo_spectrum: adds the time marginal of the map to spectrum (int64 storage of
+    uint64 [n_fbins]; created zeroed if None)."""
+    dev = map_.device.index
+    nt, nf = map_.shape
+    if spectrum is None:
+        spectrum = torch.zeros(nf, dtype=torch.int64, device=map_.device)
+    with torch.cuda.device(dev):
+        _check(_lib.bfly_pseudo_spectrum(_dev(map_, torch.int32, "map"), int(nt), int(nf),
+                                         _dev(spectrum, torch.int64, "spectrum", dev, nf), _stream(dev)),
+               "bfly_pseudo_spectrum")
+    return spectrum
 
 
 def search_host(bank: Bank, x_host, chunk_samples: int, kappa: float, samples_per_tbin: int,

@@ -324,6 +324,54 @@ int bfly_hits_map(const bfly_bank *bank, const int32_t *hit_template_dev, const 
                            (cudaStream_t)stream);
 }
 
+static int current_device_ok()
+{
+    int dev = 0;
+    BFLY_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp p;
+    BFLY_CUDA(cudaGetDeviceProperties(&p, dev));
+    if (p.major != 10) { set_error("device %d is sm_%d%d; this library is built for sm_100a only", dev, p.major, p.minor); return BFLY_EUNSUPPORTED; }
+    return BFLY_OK;
+}
+
+int bfly_time_randomize(const float *x_dev, const int32_t *perm_dev, int64_t n, float *out_dev,
+                        int32_t *bad_dev, void *stream)
+{
+    if (!x_dev || !perm_dev || !out_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n < 0 || n >= (1LL << 31)) { set_error("n must be in [0, 2^31)"); return BFLY_EINVAL; }
+    if (x_dev == out_dev) { set_error("out_dev must not alias x_dev"); return BFLY_EINVAL; }
+    int rc = current_device_ok();
+    if (rc) return rc;
+    return launch_time_randomize(x_dev, perm_dev, n, out_dev, bad_dev, (cudaStream_t)stream);
+}
+
+int bfly_coincidence(const uint32_t *map1_dev, const uint32_t *map2_dev, int32_t n_tbins,
+                     int32_t n_fbins, int32_t half_width_bins, uint32_t *co1_dev,
+                     uint32_t *co2_dev, void *stream)
+{
+    if (!map1_dev || !map2_dev || !co1_dev || !co2_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n_tbins <= 0 || n_fbins <= 0 || half_width_bins < 0) { set_error("bad map geometry or window"); return BFLY_EINVAL; }
+    if (co1_dev == map1_dev || co1_dev == map2_dev || co2_dev == map1_dev || co2_dev == map2_dev || co1_dev == co2_dev) {
+        set_error("outputs must not alias the inputs or each other");
+        return BFLY_EINVAL;
+    }
+    int rc = current_device_ok();
+    if (rc) return rc;
+    return launch_coincidence(map1_dev, map2_dev, n_tbins, n_fbins, half_width_bins, co1_dev, co2_dev,
+                              (cudaStream_t)stream);
+}
+
+int bfly_pseudo_spectrum(const uint32_t *map_dev, int32_t n_tbins, int32_t n_fbins,
+                         uint64_t *spectrum_dev, void *stream)
+{
+    if (!map_dev || !spectrum_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n_tbins <= 0 || n_fbins <= 0) { set_error("bad map geometry"); return BFLY_EINVAL; }
+    int rc = current_device_ok();
+    if (rc) return rc;
+    return launch_pseudo_spectrum(map_dev, n_tbins, n_fbins, (unsigned long long *)spectrum_dev,
+                                  (cudaStream_t)stream);
+}
+
 int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream)
 {
     if (!y_dev || !z_dev) { set_error("null pointer"); return BFLY_EINVAL; }

@@ -107,6 +107,12 @@ int launch_hits_map(const bfly_bank *b, const int32_t *hit_template, const int32
                     int64_t n_hits, int64_t lag_origin, int32_t samples_per_tbin, double f_lo,
                     double df, int32_t n_fbins, int32_t n_tbins, uint32_t *map,
                     unsigned long long *counters, cudaStream_t stream);
+int launch_time_randomize(const float *x, const int32_t *perm, int64_t n, float *out, int *bad,
+                          cudaStream_t stream);
+int launch_coincidence(const uint32_t *m1, const uint32_t *m2, int32_t n_tbins, int32_t n_fbins,
+                       int32_t w, uint32_t *c1, uint32_t *c2, cudaStream_t stream);
+int launch_pseudo_spectrum(const uint32_t *m, int32_t n_tbins, int32_t n_fbins,
+                           unsigned long long *spec, cudaStream_t stream);
 int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin, int64_t lag_end,
                     float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream);
