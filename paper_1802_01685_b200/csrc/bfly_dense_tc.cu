@@ -13,9 +13,10 @@
 // row s * 32 + r holding lag 8 r + s (rows overlap in memory; the epilogue undoes the permutation).
 // tcgen05.mma (cta_group::1, kind::f16, M = 128, N = 256, K = 16) accumulates both quadratures in
 // fp32 in tensor memory: D_c in columns 0..255, D_s in columns 256..511 (all of TMEM, one CTA per
-// SM).  Roles: warps 0-3 synthesise A (one template row per thread) and run the epilogue (one
-// TMEM lane = one template per thread: A5-A7 with no cross-thread reduction), warp 4 allocates
-// TMEM and issues the MMAs; a 3-stage full/empty mbarrier ring joins them.  A CTA owns a tile of
+// SM).  Roles: warps 0-7 synthesise A (two threads per template row, 32 samples of each K-block
+// each) and run the epilogue (one TMEM lane = one template, the two threads of a row take half of
+// the columns each: A5-A7 with one two-way merge per template), warp 8 allocates TMEM and issues
+// the MMAs; a 3-stage full/empty mbarrier ring joins them.  A CTA owns a tile of
 // 128 templates across ALL lag tiles, so the running maximum stays in registers and the only HBM
 // traffic is 32 B in and 8 B out per template.
 //
@@ -36,11 +37,13 @@ constexpr int DT_M = 128;          // templates per tile (TMEM lanes)
 constexpr int DT_N = 256;          // lags per tile (TMEM columns per quadrature)
 constexpr int DT_K = 64;           // samples per K-block (one 128-byte swizzle row of fp16)
 constexpr int DT_STAGES = 3;
-constexpr int DT_THREADS = 160;    // warps 0-3: producers + epilogue, warp 4: TMEM + MMA issue
+constexpr int DT_PRODUCER_WARPS = 8;
+constexpr int DT_THREADS = (DT_PRODUCER_WARPS + 1) * 32;   // warps 0-7: producers + epilogue, warp 8: TMEM + MMA issue
 constexpr uint32_t DT_A_BYTES = DT_M * DT_K * 2;              // 16 KB per quadrature
 constexpr uint32_t DT_B_BYTES = DT_N * DT_K * 2;              // 32 KB
 constexpr uint32_t DT_STAGE_BYTES = 2 * DT_A_BYTES + DT_B_BYTES;
-constexpr size_t DT_SMEM = (size_t)DT_STAGES * DT_STAGE_BYTES + 1024 /* alignment slack */ + 128;
+constexpr size_t DT_SMEM = (size_t)DT_STAGES * DT_STAGE_BYTES + 1024 /* alignment slack */ + 128 /* barriers */ +
+                           DT_M * 8 /* merge */;
 
 // ------------------------------------------------------------------------------------------
 // PTX wrappers (PTX ISA: mbarrier, cp.async.bulk.tensor, tcgen05)
@@ -188,14 +191,14 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
 
     if (tid == 0) {
         for (int s = 0; s < DT_STAGES; ++s) {
-            bar_init(full(s), DT_M + 1);       // 128 producer arrivals + the expect_tx arrival
+            bar_init(full(s), DT_PRODUCER_WARPS * 32 + 1);   // producer arrivals + the expect_tx arrival
             bar_init(empty(s), 1);             // one tcgen05.commit
         }
         bar_init(tmem_full, 1);
-        bar_init(tmem_empty, DT_M);
+        bar_init(tmem_empty, DT_PRODUCER_WARPS * 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 4) {                           // all of tensor memory: 512 columns
+    if (warp == DT_PRODUCER_WARPS) {           // all of tensor memory: 512 columns
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(tmem_slot) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -208,13 +211,19 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
     const int32_t n_kb = (L + DT_K - 1) / DT_K;
     const int64_t n_ttiles = (T + DT_M - 1) / DT_M;
 
-    if (warp < 4) {
-        // ===== producers (A3) and epilogue (A5-A7): thread = template row = TMEM lane =====
+    if (warp < DT_PRODUCER_WARPS) {
+        // ===== producers (A3) and epilogue (A5-A7).  Two threads per template row: thread
+        //       (row, half) synthesises samples [32 half, 32 half + 32) of every K-block and, in
+        //       the epilogue, reads TMEM lane `row`, columns [128 half, 128 half + 128) of each
+        //       quadrature (warp w may touch lanes 32 (w mod 4) .. + 31 only) =====
         int stage = 0;
         uint32_t phase = 0, tiles_done = 0;
-        const uint32_t row_off = (uint32_t)tid * 128u, row_x = (uint32_t)tid & 7u;
+        const int row = tid & (DT_M - 1), half = tid >> 7;
+        const uint32_t row_off = (uint32_t)row * 128u, row_x = (uint32_t)row & 7u;
+        unsigned long long *merge = reinterpret_cast<unsigned long long *>(dt_raw + (sbase - saddr(dt_raw)) +
+                                                                          DT_STAGES * DT_STAGE_BYTES + 128);
         for (int64_t tt = blockIdx.x; tt < n_ttiles; tt += gridDim.x) {
-            const int64_t j = tt * DT_M + tid;
+            const int64_t j = tt * DT_M + row;
             const bool valid = j < T;
             const uint64_t A = valid ? phA[j] : 0ull, Bq = valid ? phB[j] : 0ull;
             const float ic = valid ? inc2[j] : 0.0f, is = valid ? ins2[j] : 0.0f;
@@ -228,23 +237,32 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                         bar_expect_tx(full(stage), DT_B_BYTES);
                         tma_load_3d(st + 2 * DT_A_BYTES, &xmap, 0, (lt * DT_N + kb * DT_K) / 8, 0, full(stage));
                     }
-                    // phase of sample k0 and its first difference, exact to 2^-32 cycle; then
-                    // second-order recurrence in 32-bit fixed point (wrap = mod 1 cycle)
-                    const uint64_t k0 = (uint64_t)kb * DT_K;
-                    uint32_t ph = (uint32_t)((A * k0 + Bq * (k0 * k0)) >> 32);
+                    // phase of this thread's first sample and its first difference, exact to 2^-32
+                    // cycle, then a second-order recurrence in 32-bit fixed point (wrap = mod 1
+                    // cycle).  Half a cycle is added so that the bit pattern 0x3F800000 | (ph >> 9),
+                    // a float in [1, 2), minus 1.5 is the phase in [-1/2, 1/2) cycles: no
+                    // int-to-float conversion (those share the XU pipe with sin / cos).
+                    const uint64_t k0 = (uint64_t)kb * DT_K + 32u * (uint32_t)half;
+                    uint32_t ph = (uint32_t)((A * k0 + Bq * (k0 * k0)) >> 32) ^ 0x80000000u;
                     uint32_t d = (uint32_t)((A + Bq * (2ull * k0 + 1ull)) >> 32);
+                    const bool whole = valid && (int32_t)k0 + 32 <= L;
 #pragma unroll
-                    for (int c = 0; c < 8; ++c) {
+                    for (int c = 0; c < 4; ++c) {
                         uint32_t cw[4], sw[4];
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
                             float cs[2], sn[2];
 #pragma unroll
                             for (int e = 0; e < 2; ++e) {
-                                const float ang = (float)(int32_t)ph * 1.4629180792671596e-9f;   // pi 2^-31
-                                const bool on = valid && (int32_t)k0 + 8 * c + 2 * i + e < L;
-                                cs[e] = on ? __cosf(ang) : 0.0f;
-                                sn[e] = on ? __sinf(ang) : 0.0f;
+                                const float f = __uint_as_float(__funnelshift_r(ph, 0x7Fu, 9));
+                                const float ang = fmaf(f, 6.283185307179586f, -9.42477796076938f);   // 2 pi (f - 1.5)
+                                cs[e] = __cosf(ang);
+                                sn[e] = __sinf(ang);
+                                if (!whole) {
+                                    const bool on = valid && (int32_t)k0 + 8 * c + 2 * i + e < L;
+                                    cs[e] = on ? cs[e] : 0.0f;
+                                    sn[e] = on ? sn[e] : 0.0f;
+                                }
                                 ph += d;
                                 d += dd;
                             }
@@ -252,7 +270,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                             cw[i] = *reinterpret_cast<uint32_t *>(&hc);
                             sw[i] = *reinterpret_cast<uint32_t *>(&hs);
                         }
-                        const uint32_t off = row_off + (((uint32_t)c ^ row_x) << 4);
+                        const uint32_t off = row_off + (((uint32_t)(4 * half + c) ^ row_x) << 4);
                         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + off), "r"(cw[0]), "r"(cw[1]),
                                      "r"(cw[2]), "r"(cw[3]) : "memory");
                         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + DT_A_BYTES + off), "r"(sw[0]),
@@ -265,9 +283,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                 // ---- epilogue of this lag tile: column s * 32 + r holds lag 8 r + s of the tile
                 bar_wait(tmem_full, tiles_done & 1u);
                 tc_fence_after();
-                const uint32_t lane_addr = tmem_base + ((uint32_t)(warp * 32) << 16);
+                const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
 #pragma unroll 1
-                for (int s = 0; s < 8; ++s) {
+                for (int s = 4 * half; s < 4 * half + 4; ++s) {
                     uint32_t vc[32], vs[32];
                     tmem_ld32(lane_addr + (uint32_t)(s * 32), vc);
                     tmem_ld32(lane_addr + (uint32_t)(DT_N + s * 32), vs);
@@ -289,7 +307,13 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                 bar_arrive(tmem_empty);
                 ++tiles_done;
             }
-            if (valid) {
+            // the two column halves of a row meet in shared memory (the tile handshakes keep the
+            // next tile's writes behind this tile's reads)
+            if (half == 1) merge[row] = best;
+            asm volatile("bar.sync 1, %0;" ::"n"(DT_PRODUCER_WARPS * 32) : "memory");
+            if (half == 0 && valid) {
+                const unsigned long long other = merge[row];
+                best = other > best ? other : best;
                 if (best == 0ull) {
                     rho_max[j] = 0.0f;
                     arg_lag[j] = (int32_t)lag_begin;
@@ -299,7 +323,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                 }
             }
         }
-    } else if (tid == DT_M) {
+    } else if (tid == DT_PRODUCER_WARPS * 32) {
         // ===== MMA issuer (A4): one thread =====
         int stage = 0;
         uint32_t phase = 0, tiles_done = 0;
@@ -328,7 +352,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 4) {
+    if (warp == DT_PRODUCER_WARPS) {
         __syncwarp();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
     }
