@@ -58,6 +58,23 @@ def direct_form_flops(cfg, n_templates):
     return n_templates * 2 * (2 * cfg.L * cfg.n_lags)
 
 
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """The slowest rank's figure (replicas run side by side: the job ends with the last rank)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(units_per_rank: float, steps: int, seconds: float, world: int) -> float:
+    """Whole-job throughput of `world` independent replicas (replicas
+    only): the units all ranks processed over the max-over-ranks time."""
+    return world * units_per_rank * steps / seconds
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -236,12 +253,9 @@ def main():
     clocks = sampler.stop() if sampler else None
     bank.set_timing(False)
     ms = e0.elapsed_time(e1)
-    if world > 1:
-        tms = torch.tensor([ms], device=dev)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
+    ms = max_over_ranks(ms, world, dev)
     corr_step = correlations_per_step(cfg, T)
-    value = world * corr_step * args.steps / (ms * 1e-3)
+    value = replicas_value(corr_step, args.steps, ms * 1e-3, world)
 
     # ---- e2e: the same step through bfly_search_host with HOST buffers (copies inside)
     e2e = None
@@ -254,11 +268,8 @@ def main():
             bfly.search_host(bank, xh, chunk, cfg.kappa, **grid)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t
-        if world > 1:
-            tdt = torch.tensor([dt], device=dev)
-            dist.all_reduce(tdt, op=dist.ReduceOp.MAX)
-            dt = float(tdt.item())
-        e2e = {"value": world * corr_step * args.steps / dt, "unit": UNIT,
+        dt = max_over_ranks(dt, world, dev)
+        e2e = {"value": replicas_value(corr_step, args.steps, dt, world), "unit": UNIT,
                "h2d_bytes_per_step": int(x.nbytes),
                "d2h_bytes_per_step": int(T * 8 + m.numel() * 4 + 16)}
 
