@@ -270,3 +270,44 @@ def test_search_host_streaming(bfly, n_samples, chunk):
     np.testing.assert_array_equal(cnt_h, c_d.cpu().numpy().view(np.uint64))
     np.testing.assert_array_equal(rho_h, rho_n)
     np.testing.assert_array_equal(arg_h, arg_n)
+
+
+# ----------------------------------------------------------------- config 4 at full size
+def test_full_bank_config4_sampled_against_the_oracle(bfly):
+    """BASELINE.json's paper-scale bank (2^23 templates x 61441 lags) in the launch configuration
+    bench.py times (bfly_make_bank_grid, default form, persistent outputs), checked on sampled
+    templates the oracle can compute one by one (R1, R2), and against a sub-bank run of the same
+    templates bit for bit (R4: catches indexing and overflow errors at scale; templates x lags =
+    5.2e11 > 2^32).  The map is the exact histogram of the GPU's own outputs (R3 (i))."""
+    cfg = get_config(4)
+    x = make_data(cfg)
+    xd = torch.from_numpy(x).cuda()
+    full = bfly.make_bank_grid(cfg.fs_hz, cfg.L, cfg.f0_lo, cfg.f0_hi, cfg.n_f0,
+                               cfg.f1_lo, cfg.f1_hi, cfg.n_f1)
+    assert len(full) == 1 << 23
+    rho, arg = bfly.correlate(full, xd)
+    grid = default_map_grid(cfg)
+    m, c = bfly.butterfly_map(full, rho, arg, cfg.kappa, 0, **grid)
+    torch.cuda.synchronize()
+    f0a, f1a = bank_grid(cfg)
+    # the sample: the four grid corners, the last templates of the bank, the injected chirp's
+    # track, a seeded stratified draw
+    idx = np.unique(np.concatenate([sub_bank_indices(cfg, 40, seed=3, max_track=16),
+                                    [0, cfg.n_f1 - 1, len(f0a) - cfg.n_f1, len(f0a) - 1, len(f0a) - 2]]))
+    it = torch.from_numpy(idx).cuda()
+    rho_s, arg_s = rho[it].cpu().numpy(), arg[it].cpu().numpy()
+    check_values_and_argmax(x, cfg.fs_hz, cfg.L, f0a[idx], f1a[idx], rho_s, arg_s)
+    sub = bfly.make_bank(cfg.fs_hz, cfg.L, f0a[idx], f1a[idx])
+    r2, a2 = bfly.correlate(sub, xd)
+    assert np.array_equal(r2.cpu().numpy(), rho_s) and np.array_equal(a2.cpu().numpy(), arg_s)
+    # R3 (i) at full size: counters and map against the histogram of the GPU's own outputs
+    rho_n, arg_n = rho.cpu().numpy(), arg.cpu().numpy()
+    hit = rho_n > np.float32(cfg.kappa)
+    tb = arg_n[hit].astype(np.int64) // grid["samples_per_tbin"]
+    fb = np.floor((f0a[hit] - grid["f_lo_hz"]) / grid["df_hz"]).astype(np.int64)
+    ok = (tb < grid["n_tbins"]) & (fb >= 0) & (fb < grid["n_fbins"])
+    want = np.zeros((grid["n_tbins"], grid["n_fbins"]), np.uint32)
+    np.add.at(want, (tb[ok], fb[ok]), 1)
+    np.testing.assert_array_equal(m.cpu().numpy().view(np.uint32), want)
+    assert c.cpu().numpy().tolist() == [int(hit.sum()), int((~ok).sum())]
+    assert np.all((arg_n >= 0) & (arg_n < cfg.n_lags)) and np.all(np.isfinite(rho_n)) and rho_n.max() < 1.0
