@@ -179,7 +179,7 @@ def main():
                     help="0 default (= 3), 1 fp32 FFT, 2 fp32 direct, 3 tensor-core FFT, 4 dense tcgen05")
     ap.add_argument("--templates", type=int, default=0,
                     help="development only: first n templates of the bank (not a bench line)")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--cpu-seconds", type=float, default=30.0)
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
 

@@ -43,6 +43,14 @@ def lib():
                               C.c_double, C.c_double, C.c_int32, C.c_int32,
                               C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
         L.bfo_map.restype = None
+        L.bfo_template3.argtypes = [C.c_double, C.c_int, C.c_double, C.c_double, C.c_double, dp, dp]
+        L.bfo_template3.restype = None
+        L.bfo_rho_series3.argtypes = [fp, C.c_int64, C.c_double, C.c_int, C.c_double, C.c_double,
+                                      C.c_double, C.c_int64, C.c_int64, dp, dp, dp]
+        L.bfo_rho_series3.restype = None
+        L.bfo_correlate3.argtypes = [fp, C.c_int64, C.c_double, C.c_int, C.c_int64, dp, dp, dp,
+                                     C.c_int64, C.c_int64, dp, ip, C.c_int]
+        L.bfo_correlate3.restype = C.c_int
         L.bfo_sigma.argtypes = [fp, C.c_int64, C.c_double, C.c_int, C.c_double, C.c_double]
         L.bfo_sigma.restype = C.c_double
         L.bfo_tails.argtypes = [fp, C.c_int64, C.c_double, C.c_int, C.c_int64, dp, dp, C.c_int64,
@@ -73,12 +81,12 @@ def max_threads() -> int:
     return int(lib().bfo_max_threads())
 
 
-def template(fs, L, f0, f1):
-    """(hc, hs): un-normalised cosine and sine templates, float64[L] each."""
+def template(fs, L, f0, f1, f2=0.0):
+    """(hc, hs): un-normalised cosine and sine templates, float64[L] each (f2: reading N1)."""
     hc = np.empty(L, np.float64)
     hs = np.empty(L, np.float64)
-    lib().bfo_template(float(fs), int(L), float(f0), float(f1), _p(hc, C.c_double),
-                       _p(hs, C.c_double))
+    lib().bfo_template3(float(fs), int(L), float(f0), float(f1), float(f2), _p(hc, C.c_double),
+                        _p(hs, C.c_double))
     return hc, hs
 
 
@@ -110,7 +118,7 @@ def sliding_n2(x, L, lag_begin=0, lag_end=None):
     return out
 
 
-def rho_series(x, fs, L, f0, f1, lag_begin=0, lag_end=None, components=False):
+def rho_series(x, fs, L, f0, f1, lag_begin=0, lag_end=None, components=False, f2=0.0):
     """rho(tau) of one template over lag_begin <= tau < lag_end (float64)."""
     x = _f32(x)
     lag_end = len(x) - L + 1 if lag_end is None else lag_end
@@ -124,12 +132,12 @@ def rho_series(x, fs, L, f0, f1, lag_begin=0, lag_end=None, components=False):
         cp, sp = _p(c, C.c_double), _p(s, C.c_double)
     else:
         cp = sp = None
-    lib().bfo_rho_series(_p(x, C.c_float), len(x), float(fs), int(L), float(f0), float(f1),
-                         int(lag_begin), int(lag_end), _p(rho, C.c_double), cp, sp)
+    lib().bfo_rho_series3(_p(x, C.c_float), len(x), float(fs), int(L), float(f0), float(f1),
+                          float(f2), int(lag_begin), int(lag_end), _p(rho, C.c_double), cp, sp)
     return (rho, c, s) if components else rho
 
 
-def correlate(x, fs, L, f0, f1, lag_begin=0, lag_end=None, n_threads=0):
+def correlate(x, fs, L, f0, f1, lag_begin=0, lag_end=None, n_threads=0, f2=None):
     """(rho_max float64[T], arg_lag int32[T]) over lag_begin <= tau < lag_end."""
     x = _f32(x)
     f0, f1 = _f64(f0), _f64(f1)
@@ -139,10 +147,15 @@ def correlate(x, fs, L, f0, f1, lag_begin=0, lag_end=None, n_threads=0):
     T = len(f0)
     rho_max = np.empty(T, np.float64)
     arg = np.empty(T, np.int32)
-    rc = lib().bfo_correlate(_p(x, C.c_float), len(x), float(fs), int(L), T,
-                             _p(f0, C.c_double), _p(f1, C.c_double), int(lag_begin),
-                             int(lag_end), _p(rho_max, C.c_double), _p(arg, C.c_int32),
-                             int(n_threads))
+    if f2 is not None:
+        f2 = _f64(f2)
+        if f2.shape != f0.shape:
+            raise ValueError("f2 must have the shape of f0")
+    rc = lib().bfo_correlate3(_p(x, C.c_float), len(x), float(fs), int(L), T,
+                              _p(f0, C.c_double), _p(f1, C.c_double),
+                              _p(f2, C.c_double) if f2 is not None else None, int(lag_begin),
+                              int(lag_end), _p(rho_max, C.c_double), _p(arg, C.c_int32),
+                              int(n_threads))
     if rc < 0:
         raise ValueError("bfo_correlate: bad arguments")
     return rho_max, arg

@@ -54,6 +54,23 @@ void bfo_template(double fs, int L, double f0, double f1, double *hc, double *hs
     }
 }
 
+/* N1 (descending chirps that settle
+ * towards a late-time plateau; the paper gives no waveform): the non-linear family is the chirp
+ * with a constant second frequency derivative f2 [Hz/s^2],
+ *   f(t) = f0 + f1 t + 1/2 f2 t^2,   phi_k = 2 pi (f0 t_k + 1/2 f1 t_k^2 + 1/6 f2 t_k^3),
+ * which represents an exponentially settling chirp f_inf + D exp(-t/tc) over one template by its
+ * frequency, slope and curvature at the template's first sample.  f2 = 0 is bfo_template. */
+void bfo_template3(double fs, int L, double f0, double f1, double f2, double *hc, double *hs)
+{
+    if (f2 == 0.0) { bfo_template(fs, L, f0, f1, hc, hs); return; }
+    for (int k = 0; k < L; ++k) {
+        double t = (double)k / fs;
+        double phi = 2.0 * BFO_PI * (f0 * t + 0.5 * f1 * t * t + f2 * t * t * t / 6.0);
+        hc[k] = cos(phi);
+        hs[k] = sin(phi);
+    }
+}
+
 /* C2 ("each unit-L2-normalized", BASELINE.json configs[0]): the L2 norms of the
  * cosine and of the sine template, taken separately. */
 void bfo_template_norms(int L, const double *hc, const double *hs, double *nc, double *ns)
@@ -143,15 +160,26 @@ static void bfo_dots_run(const double *restrict xd, int L, const double *restric
 
 /* rho_j(tau) of ONE template for lag_begin <= tau < lag_end (needed for the argmax
  * rule and the pins).  c_out / s_out (optional) receive c/||x_tau||, s/||x_tau||. */
+void bfo_rho_series3(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
+                     double f2, int64_t lag_begin, int64_t lag_end, double *rho, double *c_out,
+                     double *s_out);
 void bfo_rho_series(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
                     int64_t lag_begin, int64_t lag_end, double *rho, double *c_out, double *s_out)
+{
+    bfo_rho_series3(x, n_samples, fs, L, f0, f1, 0.0, lag_begin, lag_end, rho, c_out, s_out);
+}
+
+/* The same for a template of the non-linear family (N1). */
+void bfo_rho_series3(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
+                     double f2, int64_t lag_begin, int64_t lag_end, double *rho, double *c_out,
+                     double *s_out)
 {
     double *xd = (double *)malloc(sizeof(double) * (size_t)n_samples);
     for (int64_t i = 0; i < n_samples; ++i) xd[i] = (double)x[i];
     double *hc = (double *)malloc(sizeof(double) * (size_t)L);
     double *hs = (double *)malloc(sizeof(double) * (size_t)L);
     double nc, ns;
-    bfo_template(fs, L, f0, f1, hc, hs);
+    bfo_template3(fs, L, f0, f1, f2, hc, hs);
     bfo_template_norms(L, hc, hs, &nc, &ns);
     double c[BFO_RUN], s[BFO_RUN];
     for (int64_t tau0 = lag_begin; tau0 < lag_end; tau0 += BFO_RUN) {
@@ -183,9 +211,21 @@ void bfo_rho_series(const float *x, int64_t n_samples, double fs, int L, double 
  * lags only (C5): requires 0 <= lag_begin <= lag_end <= n_samples - L + 1.
  * Templates are independent; OpenMP runs them on n_threads threads (0 = default).
  * Returns the number of threads used, or -1 on bad arguments. */
+int bfo_correlate3(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
+                   const double *f0, const double *f1, const double *f2, int64_t lag_begin,
+                   int64_t lag_end, double *rho_max, int32_t *arg_lag, int n_threads);
 int bfo_correlate(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
                   const double *f0, const double *f1, int64_t lag_begin, int64_t lag_end,
                   double *rho_max, int32_t *arg_lag, int n_threads)
+{
+    return bfo_correlate3(x, n_samples, fs, L, n_templates, f0, f1, 0, lag_begin, lag_end, rho_max,
+                          arg_lag, n_threads);
+}
+
+/* The same with a per-template second frequency derivative f2 (N1); f2 == NULL means 0. */
+int bfo_correlate3(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
+                   const double *f0, const double *f1, const double *f2, int64_t lag_begin,
+                   int64_t lag_end, double *rho_max, int32_t *arg_lag, int n_threads)
 {
     if (L < 1 || n_samples < L || lag_begin < 0 || lag_end < lag_begin ||
         lag_end > n_samples - L + 1)
@@ -210,7 +250,7 @@ int bfo_correlate(const float *x, int64_t n_samples, double fs, int L, int64_t n
 #pragma omp for schedule(dynamic, 1)
         for (int64_t j = 0; j < n_templates; ++j) {
             double nc, ns;
-            bfo_template(fs, L, f0[j], f1[j], hc, hs);
+            bfo_template3(fs, L, f0[j], f1[j], f2 ? f2[j] : 0.0, hc, hs);
             bfo_template_norms(L, hc, hs, &nc, &ns);
             double best = -1.0;
             int64_t arg = lag_begin;
