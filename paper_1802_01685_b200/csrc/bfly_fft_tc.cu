@@ -501,15 +501,27 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             const float4 ra = __ldg(rp), rb4 = __ldg(rp + 1);
             const float2 rr[4] = {make_float2(ra.x, ra.y), make_float2(ra.z, ra.w),
                                   make_float2(rb4.x, rb4.y), make_float2(rb4.z, rb4.w)};
+            float2 qs4[4];
+            float qmax = 0.0f;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 cpair z, zu;
                 chain2<false, TC_HALF>(k, rbuf, 4 * w + i, lane, z, zu, nowu);
                 const float2 q = __fmul2_rn(__ffma2_rn(z.i, z.i, __fmul2_rn(z.r, z.r)), rr[i]);
                 if (TAILS) {
+                    qs4[i] = q;
+                    qmax = fmaxf(qmax, fmaxf(q.x, q.y));
+                } else {
+                    if (q.x > best) { best = q.x; code = 8 * b + 2 * i; }
+                    if (q.y > best) { best = q.y; code = 8 * b + 2 * i + 1; }
+                }
+            }
+            if (TAILS && qmax > thr) {                 // rare: at least one of this thread's 8 lags is a hit
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
-                        const float qe = e ? q.y : q.x;
+                        const float qe = e ? qs4[i].y : qs4[i].x;
                         if (qe > thr) {
                             const unsigned long long at = atomicAdd(ta.n_hits, 1ull);
                             if (at < (unsigned long long)ta.capacity) {
@@ -519,9 +531,6 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                             }
                         }
                     }
-                } else {
-                    if (q.x > best) { best = q.x; code = 8 * b + 2 * i; }
-                    if (q.y > best) { best = q.y; code = 8 * b + 2 * i + 1; }
                 }
             }
         }
