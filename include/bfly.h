@@ -86,6 +86,20 @@ int bfly_make_bank(double fs_hz, int32_t L, int64_t n_templates,
                    const double *f0_hz, const double *f1_hzps,
                    int device, bfly_bank **out_bank);
 
+/* The non-linear family (descending chirps that
+ * settle towards a late-time frequency; the paper gives no waveform; reading N1 of DESIGN.md):
+ * templates with a constant second frequency derivative f2 [Hz/s^2],
+ *     f(t) = f0 + f1 t + f2 t^2 / 2,     phi_k = 2 pi (f0 t_k + f1 t_k^2 / 2 + f2 t_k^3 / 6),
+ * which carry an exponentially settling chirp f_inf + D exp(-t / tc) over one template by its
+ * frequency, slope and curvature at the template's first sample.  f2_hzps2: HOST, n_templates
+ * float64, or NULL for all zero (then identical to bfly_make_bank).  Every other call works on
+ * such a bank unchanged; bfly_butterfly_map bins by f0 as before. */
+int bfly_make_bank3(double fs_hz, int32_t L, int64_t n_templates,
+                    const double *f0_hz, const double *f1_hzps, const double *f2_hzps2,
+                    int device, bfly_bank **out_bank);
+/* f2 of templates [first, first + count) to a HOST float64 array.  Synchronous. */
+int bfly_bank_get_f2(const bfly_bank *bank, int64_t first, int64_t count, double *f2_hzps2);
+
 /* Convenience: inclusive uniform grids f0 = f0_lo + i (f0_hi - f0_lo)/(n_f0 - 1) (likewise
  * f1), evaluated in float64 exactly like numpy.linspace; template j = i_f0 * n_f1 + i_f1. */
 int bfly_make_bank_grid(double fs_hz, int32_t L,

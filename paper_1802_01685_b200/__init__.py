@@ -41,6 +41,8 @@ def _load():
     lib.bfly_last_error.restype = C.c_char_p
     lib.bfly_last_error.argtypes = []
     lib.bfly_make_bank.argtypes = [f64, i32, i64, vp, vp, C.c_int, C.POINTER(vp)]
+    lib.bfly_make_bank3.argtypes = [f64, i32, i64, vp, vp, vp, C.c_int, C.POINTER(vp)]
+    lib.bfly_bank_get_f2.argtypes = [vp, i64, i64, vp]
     lib.bfly_make_bank_grid.argtypes = [f64, i32, f64, f64, i32, f64, f64, i32, C.c_int,
                                         C.POINTER(vp)]
     lib.bfly_free_bank.argtypes = [vp]
@@ -67,7 +69,8 @@ def _load():
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
                  "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
                  "bfly_search_host", "bfly_debug_fft_tc", "bfly_tails", "bfly_hits_map",
-                 "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum"):
+                 "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum",
+                 "bfly_make_bank3", "bfly_bank_get_f2"):
         getattr(lib, name).restype = C.c_int
     return lib, path
 
@@ -135,6 +138,12 @@ class Bank:
                                   a.ctypes.data, b.ctypes.data), "bfly_bank_get")
         return f0, f1, a, b
 
+    def get_f2(self, first: int = 0, count: int | None = None):
+        count = len(self) - first if count is None else count
+        f2 = np.empty(count, np.float64)
+        _check(_lib.bfly_bank_get_f2(self._h, first, count, f2.ctypes.data), "bfly_bank_get_f2")
+        return f2
+
     def set_timing(self, enable: bool):
         _check(_lib.bfly_bank_set_timing(self._h, int(bool(enable))), "bfly_bank_set_timing")
 
@@ -148,14 +157,23 @@ class Bank:
         _check(_lib.bfly_bank_reserve(self._h, int(max_n_samples)), "bfly_bank_reserve")
 
 
-def make_bank(fs_hz: float, L: int, f0_hz, f1_hzps, device: int = 0) -> Bank:
+def make_bank(fs_hz: float, L: int, f0_hz, f1_hzps, device: int = 0, f2_hzps2=None) -> Bank:
+    """bfly_make_bank, or bfly_make_bank3 when f2_hzps2 (the second frequency derivative of the
+    non-linear family) is given."""
     f0 = np.ascontiguousarray(f0_hz, dtype=np.float64)
     f1 = np.ascontiguousarray(f1_hzps, dtype=np.float64)
     if f0.ndim != 1 or f0.shape != f1.shape:
         raise ValueError("f0 and f1 must be 1-D and of equal length")
     h = C.c_void_p()
-    _check(_lib.bfly_make_bank(float(fs_hz), int(L), f0.size, f0.ctypes.data, f1.ctypes.data,
-                               int(device), C.byref(h)), "bfly_make_bank")
+    if f2_hzps2 is None:
+        _check(_lib.bfly_make_bank(float(fs_hz), int(L), f0.size, f0.ctypes.data, f1.ctypes.data,
+                                   int(device), C.byref(h)), "bfly_make_bank")
+    else:
+        f2 = np.ascontiguousarray(f2_hzps2, dtype=np.float64)
+        if f2.shape != f0.shape:
+            raise ValueError("f2 must have the shape of f0")
+        _check(_lib.bfly_make_bank3(float(fs_hz), int(L), f0.size, f0.ctypes.data, f1.ctypes.data,
+                                    f2.ctypes.data, int(device), C.byref(h)), "bfly_make_bank3")
     return Bank(h, int(device), fs_hz, L)
 
 

@@ -109,7 +109,7 @@ void bfly_free_bank(bfly_bank *b)
 {
     if (!b) return;
     cudaSetDevice(b->device);
-    cudaFree(b->f0); cudaFree(b->f1); cudaFree(b->phA); cudaFree(b->phB);
+    cudaFree(b->f0); cudaFree(b->f1); cudaFree(b->f2); cudaFree(b->phA); cudaFree(b->phB); cudaFree(b->phC);
     cudaFree(b->inc2); cudaFree(b->ins2); cudaFree(b->rn2); cudaFree(b->xspec);
     cudaFree(b->xh); cudaFree(b->rn2p); cudaFree(b->qs);
     cudaFree(b->ys); cudaFree(b->rn2s); cudaFree(b->maxbits); cudaFree(b->racf); cudaFree(b->wspec);
@@ -125,14 +125,20 @@ int64_t bfly_bank_size(const bfly_bank *b) { return b ? b->T : -1; }
 int bfly_make_bank(double fs_hz, int32_t L, int64_t n_templates, const double *f0_hz,
                    const double *f1_hzps, int device, bfly_bank **out_bank)
 {
+    return bfly_make_bank3(fs_hz, L, n_templates, f0_hz, f1_hzps, nullptr, device, out_bank);
+}
+
+int bfly_make_bank3(double fs_hz, int32_t L, int64_t n_templates, const double *f0_hz,
+                    const double *f1_hzps, const double *f2_hzps2, int device, bfly_bank **out_bank)
+{
     if (!out_bank || !f0_hz || !f1_hzps) { set_error("null pointer"); return BFLY_EINVAL; }
     if (!(fs_hz > 0.0) || !std::isfinite(fs_hz)) { set_error("fs must be finite and > 0"); return BFLY_EINVAL; }
     if (L < 2) { set_error("L must be >= 2"); return BFLY_EINVAL; }
     if (L > FFT_MAX_L) { set_error("L = %d exceeds the supported maximum %d", L, FFT_MAX_L); return BFLY_ERANGE; }
     if (n_templates < 1) { set_error("n_templates must be >= 1"); return BFLY_EINVAL; }
     for (int64_t j = 0; j < n_templates; ++j)
-        if (!std::isfinite(f0_hz[j]) || !std::isfinite(f1_hzps[j])) {
-            set_error("template %lld has a non-finite f0 or f1", (long long)j);
+        if (!std::isfinite(f0_hz[j]) || !std::isfinite(f1_hzps[j]) || (f2_hzps2 && !std::isfinite(f2_hzps2[j]))) {
+            set_error("template %lld has a non-finite f0, f1 or f2", (long long)j);
             return BFLY_EINVAL;
         }
     int sms = 0;
@@ -149,6 +155,8 @@ int bfly_make_bank(double fs_hz, int32_t L, int64_t n_templates, const double *f
     BANK_TRY(cudaMalloc((void **)&b->f1, T * sizeof(double)));
     BANK_TRY(cudaMalloc((void **)&b->phA, T * sizeof(uint64_t)));
     BANK_TRY(cudaMalloc((void **)&b->phB, T * sizeof(uint64_t)));
+    BANK_TRY(cudaMalloc((void **)&b->f2, T * sizeof(double)));
+    BANK_TRY(cudaMalloc((void **)&b->phC, T * sizeof(uint64_t)));
     BANK_TRY(cudaMalloc((void **)&b->inc2, T * sizeof(float)));
     BANK_TRY(cudaMalloc((void **)&b->ins2, T * sizeof(float)));
     BANK_TRY(cudaMalloc((void **)&b->packed, T * sizeof(unsigned long long)));
@@ -157,6 +165,8 @@ int bfly_make_bank(double fs_hz, int32_t L, int64_t n_templates, const double *f
     BANK_TRY(cudaMalloc((void **)&b->cnt_stage, 2 * sizeof(unsigned long long)));
     BANK_TRY(cudaMemcpy(b->f0, f0_hz, T * sizeof(double), cudaMemcpyHostToDevice));
     BANK_TRY(cudaMemcpy(b->f1, f1_hzps, T * sizeof(double), cudaMemcpyHostToDevice));
+    if (f2_hzps2) { BANK_TRY(cudaMemcpy(b->f2, f2_hzps2, T * sizeof(double), cudaMemcpyHostToDevice)); }
+    else { BANK_TRY(cudaMemset(b->f2, 0, T * sizeof(double))); }
 #undef BANK_TRY
     rc = launch_bank_params(b, 0);
     if (rc == BFLY_OK) {
@@ -204,6 +214,15 @@ int bfly_bank_get(const bfly_bank *b, int64_t first, int64_t count, double *f0_h
     if (f1_hzps) BFLY_CUDA(cudaMemcpy(f1_hzps, b->f1 + first, n * sizeof(double), cudaMemcpyDeviceToHost));
     if (inv_nc2) BFLY_CUDA(cudaMemcpy(inv_nc2, b->inc2 + first, n * sizeof(float), cudaMemcpyDeviceToHost));
     if (inv_ns2) BFLY_CUDA(cudaMemcpy(inv_ns2, b->ins2 + first, n * sizeof(float), cudaMemcpyDeviceToHost));
+    return BFLY_OK;
+}
+
+int bfly_bank_get_f2(const bfly_bank *b, int64_t first, int64_t count, double *f2_hzps2)
+{
+    if (!b || !f2_hzps2) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (first < 0 || count < 0 || first + count > b->T) { set_error("template range outside the bank"); return BFLY_EINVAL; }
+    BFLY_CUDA(cudaSetDevice(b->device));
+    BFLY_CUDA(cudaMemcpy(f2_hzps2, b->f2 + first, (size_t)count * sizeof(double), cudaMemcpyDeviceToHost));
     return BFLY_OK;
 }
 

@@ -12,8 +12,10 @@ namespace bfly {
 __global__ void __launch_bounds__(256) bank_params_kernel(int64_t T, int32_t L, double fs,
                                                           const double *__restrict__ f0,
                                                           const double *__restrict__ f1,
+                                                          const double *__restrict__ f2,
                                                           uint64_t *__restrict__ phA,
                                                           uint64_t *__restrict__ phB,
+                                                          uint64_t *__restrict__ phC,
                                                           float *__restrict__ inc2,
                                                           float *__restrict__ ins2)
 {
@@ -23,15 +25,18 @@ __global__ void __launch_bounds__(256) bank_params_kernel(int64_t T, int32_t L, 
     // cycles per sample and per sample^2, reduced mod 1, as 2^-64 fixed point
     double a = f0[j] / fs;
     double b = 0.5 * f1[j] / (fs * fs);
+    double c3 = f2[j] / (6.0 * fs * fs * fs);        // cycles per sample^3 (reading N1)
+    c3 -= floor(c3 + 0.5);
     a -= floor(a);                       // [0, 1]  (1.0 only by rounding of a tiny negative a)
     if (a >= 1.0) a = 0.0;
     b -= floor(b + 0.5);                 // [-0.5, 0.5)
     // scaling by 2^64 is exact; a < 1 and |b| <= 0.5 keep both conversions in range
     const uint64_t A = __double2ull_rn(a * 18446744073709551616.0);
     const uint64_t B = (uint64_t)__double2ll_rn(b * 18446744073709551616.0);
+    const uint64_t C = (uint64_t)__double2ll_rn(c3 * 18446744073709551616.0);
     double sc = 0.0, ss = 0.0;
     for (int32_t k = lane; k < L; k += 32) {
-        const uint64_t ph = A * (uint64_t)k + B * ((uint64_t)k * (uint64_t)k);
+        const uint64_t ph = template_phase(A, B, C, (uint64_t)k);
         // signed fraction of a turn in [-0.5, 0.5): angle = 2 pi * fr
         const double fr = (double)(int64_t)ph * 5.421010862427522e-20;   // 2^-64
         double s, c;
@@ -46,6 +51,7 @@ __global__ void __launch_bounds__(256) bank_params_kernel(int64_t T, int32_t L, 
     if (lane == 0) {
         phA[j] = A;
         phB[j] = B;
+        phC[j] = C;
         inc2[j] = sc > 0.0 ? (float)(1.0 / sc) : 0.0f;
         ins2[j] = ss > 0.0 ? (float)(1.0 / ss) : 0.0f;
     }
@@ -57,7 +63,8 @@ int launch_bank_params(bfly_bank *b, cudaStream_t stream)
     const int64_t blocks = (b->T + warps - 1) / warps;
     if (blocks >= (1LL << 31)) { set_error("bank too large"); return BFLY_ERANGE; }
     bank_params_kernel<<<(unsigned)blocks, warps * 32, 0, stream>>>(b->T, b->L, b->fs, b->f0, b->f1,
-                                                                    b->phA, b->phB, b->inc2, b->ins2);
+                                                                    b->f2, b->phA, b->phB, b->phC,
+                                                                    b->inc2, b->ins2);
     count_launch();
     BFLY_CUDA(cudaGetLastError());
     return BFLY_OK;

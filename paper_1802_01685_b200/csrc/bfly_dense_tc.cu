@@ -176,7 +176,7 @@ __global__ void dense_prep_kernel(const float *__restrict__ x, int64_t n_samples
 __global__ void __launch_bounds__(DT_THREADS, 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                 const uint64_t *__restrict__ phA, const uint64_t *__restrict__ phB,
-                const float *__restrict__ inc2, const float *__restrict__ ins2,
+                const uint64_t *__restrict__ phC, const float *__restrict__ inc2, const float *__restrict__ ins2,
                 const float *__restrict__ rn2s, int64_t n_lags, int32_t n_lag_tiles,
                 int64_t lag_begin, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
 {
@@ -225,9 +225,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
         for (int64_t tt = blockIdx.x; tt < n_ttiles; tt += gridDim.x) {
             const int64_t j = tt * DT_M + row;
             const bool valid = j < T;
-            const uint64_t A = valid ? phA[j] : 0ull, Bq = valid ? phB[j] : 0ull;
+            const uint64_t A = valid ? phA[j] : 0ull, Bq = valid ? phB[j] : 0ull, Cq = valid ? phC[j] : 0ull;
             const float ic = valid ? inc2[j] : 0.0f, is = valid ? ins2[j] : 0.0f;
-            const uint32_t dd = (uint32_t)((2ull * Bq) >> 32);
+            const uint32_t d3 = (uint32_t)((6ull * Cq) >> 32);     // third difference of the phase (reading N1)
             unsigned long long best = 0ull;
             for (int32_t lt = 0; lt < n_lag_tiles; ++lt) {
                 for (int32_t kb = 0; kb < n_kb; ++kb) {
@@ -237,14 +237,17 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                         bar_expect_tx(full(stage), DT_B_BYTES);
                         tma_load_3d(st + 2 * DT_A_BYTES, &xmap, 0, (lt * DT_N + kb * DT_K) / 8, 0, full(stage));
                     }
-                    // phase of this thread's first sample and its first difference, exact to 2^-32
-                    // cycle, then a second-order recurrence in 32-bit fixed point (wrap = mod 1
-                    // cycle).  Half a cycle is added so that the bit pattern 0x3F800000 | (ph >> 9),
+                    // phase of this thread's first sample and its first two differences, exact to
+                    // 2^-32 cycle, then a third-order recurrence in 32-bit fixed point (wrap = mod 1
+                    // cycle; the third difference 6 C is constant, 0 for a linear chirp).  Half a cycle is added so that the bit pattern 0x3F800000 | (ph >> 9),
                     // a float in [1, 2), minus 1.5 is the phase in [-1/2, 1/2) cycles: no
                     // int-to-float conversion (those share the XU pipe with sin / cos).
                     const uint64_t k0 = (uint64_t)kb * DT_K + 32u * (uint32_t)half;
-                    uint32_t ph = (uint32_t)((A * k0 + Bq * (k0 * k0)) >> 32) ^ 0x80000000u;
-                    uint32_t d = (uint32_t)((A + Bq * (2ull * k0 + 1ull)) >> 32);
+                    const uint64_t p0 = template_phase(A, Bq, Cq, k0), p1 = template_phase(A, Bq, Cq, k0 + 1),
+                                   p2 = template_phase(A, Bq, Cq, k0 + 2);
+                    uint32_t ph = (uint32_t)(p0 >> 32) ^ 0x80000000u;
+                    uint32_t d = (uint32_t)((p1 - p0) >> 32);
+                    uint32_t dd = (uint32_t)((p2 - 2ull * p1 + p0) >> 32);
                     const bool whole = valid && (int32_t)k0 + 32 <= L;
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
@@ -265,6 +268,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                                 }
                                 ph += d;
                                 d += dd;
+                                dd += d3;
                             }
                             __half2 hc = __floats2half2_rn(cs[0], cs[1]), hs = __floats2half2_rn(sn[0], sn[1]);
                             cw[i] = *reinterpret_cast<uint32_t *>(&hc);
@@ -432,7 +436,7 @@ int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag
     const int64_t ctas = std::min<int64_t>(n_ttiles, b->sm_count);
     core_timer_start(b, stream);
     dense_tc_kernel<<<(unsigned)ctas, DT_THREADS, DT_SMEM, stream>>>(
-        map, b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, b->rn2s, n_lags, (int32_t)n_lag_tiles, lag_begin,
+        map, b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->rn2s, n_lags, (int32_t)n_lag_tiles, lag_begin,
         rho_max, arg_lag);
     core_timer_stop(b, stream);
     count_launch();

@@ -61,7 +61,8 @@ data_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_
 template <int SV>
 __global__ void __launch_bounds__(NT, 1)
 fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
-                     const uint64_t *__restrict__ phB, const float *__restrict__ inc2,
+                     const uint64_t *__restrict__ phB, const uint64_t *__restrict__ phC,
+                     const float *__restrict__ inc2,
                      const float *__restrict__ ins2, const float2 *__restrict__ xspec,
                      const float *__restrict__ rn2, int64_t lag_begin, int64_t n_lags, int32_t V,
                      int32_t n_blocks, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
@@ -74,13 +75,13 @@ fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 
     for (int64_t j = blockIdx.x; j < T; j += gridDim.x) {
         // ---- A3: synthesise g[n] = exp(-i phi_n), n = t + 512 s < L, and transform it
-        const uint64_t A = phA[j], Bq = phB[j];
+        const uint64_t A = phA[j], Bq = phB[j], Cq = phC[j];
         float2 G[PTS];
 #pragma unroll
         for (int s = 0; s < PTS; ++s) {
             const int n = t + NT * s;
             float sn = 0.0f, cs = 0.0f;
-            if (n < L) template_sincos(A, Bq, (uint32_t)n, &sn, &cs);
+            if (n < L) template_sincos(A, Bq, Cq, (uint32_t)n, &sn, &cs);
             G[s] = make_float2(cs, -sn);
         }
         fft8192(G, sm, t);
@@ -174,7 +175,7 @@ int launch_fft(const bfly_bank *b, const float *x, int64_t n_samples, int64_t la
     const int sv = (V + NT - 1) / NT;
 #define BFLY_FFT_LAUNCH(SV_)                                                                        \
     fft_correlate_kernel<SV_><<<(unsigned)ctas, NT, FFT_SMEM, stream>>>(                             \
-        b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, b->xspec, b->rn2, lag_begin, n_lags, V,       \
+        b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->xspec, b->rn2, lag_begin, n_lags, V, \
         (int32_t)n_blocks, rho_max, arg_lag)
     if (sv <= 9) BFLY_FFT_LAUNCH(9);
     else if (sv <= 13) BFLY_FFT_LAUNCH(13);

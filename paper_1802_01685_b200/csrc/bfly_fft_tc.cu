@@ -284,7 +284,8 @@ struct TailArgs {
 template <bool TAILS>
 __global__ void __launch_bounds__(NT, 1)
 tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
-                    const uint64_t *__restrict__ phB, const float *__restrict__ inc2,
+                    const uint64_t *__restrict__ phB, const uint64_t *__restrict__ phC,
+                    const float *__restrict__ inc2,
                     const float *__restrict__ ins2, const uint4 *__restrict__ xh,
                     const float4 *__restrict__ rn2p, const float *__restrict__ x,
                     const float *__restrict__ rn2, int64_t lag_begin, int32_t n_blocks,
@@ -339,7 +340,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         // ---- A3: synthesise g[n] = cos phi_n - i r sin phi_n, r = ||cos phi|| / ||sin phi||,
         //      n = 1024 a + 128 g + 16 c + d' < L, as the operand fragments of pass A (so that
         //      |z|^2 / ||cos phi||^2 is the quadrature sum); direct sums for the tail lags
-        const uint64_t A = phA[j], Bq = phB[j];
+        const uint64_t A = phA[j], Bq = phB[j], Cq = phC[j];
         const uint32_t Ahi = (uint32_t)(A >> 32), Alo = (uint32_t)A;
         const uint32_t Bhi = (uint32_t)(Bq >> 32), Blo = (uint32_t)Bq;
         const float ic = inc2[j], rq = sqrtf(ins2[j] / ic);   // ic > 0: cos phi_0 = 1
@@ -357,7 +358,14 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const int n = 1024 * (2 * t + e) + 128 * g + 16 * c + dp;
                     cs[e] = sn[e] = 0.0f;
                     if (n < L) {
-                        synth_sincos(Ahi, Alo, Bhi, Blo, (uint32_t)n, &sn[e], &cs[e]);
+                        if (Cq == 0ull) {            // linear chirp (uniform over the CTA)
+                            synth_sincos(Ahi, Alo, Bhi, Blo, (uint32_t)n, &sn[e], &cs[e]);
+                        } else {                     // reading N1: cubic phase, full 64-bit Horner
+                            const uint32_t ph = (uint32_t)(template_phase(A, Bq, Cq, (uint64_t)n) >> 32);
+                            const float ang = (float)(int32_t)ph * 1.4629180792671596e-9f;
+                            sn[e] = __sinf(ang);
+                            cs[e] = __cosf(ang);
+                        }
                         sn[e] *= rq;
                         if (n_tail > 0) {
                             const float xv = sm.xt[xt_slot(n)];
@@ -680,12 +688,12 @@ static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_sample
     core_timer_start(b, stream);
     if (tails)
         tc_correlate_kernel<true><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
-            b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
+            b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
             reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
             rho_max, arg_lag, *tails);
     else
         tc_correlate_kernel<false><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
-            b->T, b->L, b->phA, b->phB, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
+            b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
             reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
             rho_max, arg_lag, TailArgs{});
     core_timer_stop(b, stream);

@@ -16,8 +16,10 @@ struct bfly_bank {
     // per-template parameters (device, struct of arrays; A1)
     double *f0;      // Hz
     double *f1;      // Hz/s
+    double *f2;      // Hz/s^2 (reading N1: the non-linear family; all zero for a linear bank)
     uint64_t *phA;   // f0/fs            in units of 2^-64 cycles per sample
     uint64_t *phB;   // f1/(2 fs^2)      in units of 2^-64 cycles per sample^2
+    uint64_t *phC;   // f2/(6 fs^3)      in units of 2^-64 cycles per sample^3
     float *inc2;     // 1 / ||cos phi||^2 (0 if the norm is 0)
     float *ins2;     // 1 / ||sin phi||^2
     // workspace (grown by bfly_bank_reserve / on demand)
@@ -117,11 +119,16 @@ int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag
                     float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream);
 
-// Template phase in cycles, as a 64-bit fixed-point fraction: phi_k/2pi mod 1 = (A k + B k^2) 2^-64.
-__device__ __forceinline__ void template_sincos(uint64_t A, uint64_t B, uint32_t k, float *s,
+// Template phase in cycles, as a 64-bit fixed-point fraction:
+// phi_k/2pi mod 1 = (A k + B k^2 + C k^3) 2^-64 (Horner, modulo 2^64: the wrap is the mod 1).
+__device__ __forceinline__ uint64_t template_phase(uint64_t A, uint64_t B, uint64_t C, uint64_t k)
+{
+    return ((C * k + B) * k + A) * k;
+}
+__device__ __forceinline__ void template_sincos(uint64_t A, uint64_t B, uint64_t C, uint32_t k, float *s,
                                                 float *c)
 {
-    uint64_t ph = A * (uint64_t)k + B * ((uint64_t)k * (uint64_t)k);
+    uint64_t ph = template_phase(A, B, C, k);
     // top 32 bits as a signed fraction of a half-turn: angle = pi * v, v in [-1, 1)
     float v = (float)(int32_t)(uint32_t)(ph >> 32) * 4.656612873077393e-10f;  // 2^-31
     sincospif(v, s, c);

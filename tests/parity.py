@@ -17,14 +17,14 @@ KAPPA_BAND = 2e-4    # R3
 
 
 def check_values_and_argmax(x, fs, L, f0, f1, rho_gpu, arg_gpu, lag_begin=0, lag_end=None,
-                            oracle_result=None):
+                            oracle_result=None, f2=None):
     """R1, R2a, R2b for every template.  Returns (rho_oracle, arg_oracle, exempt) where
     exempt[j] is True when template j's argmax is not unique to within GAP_STRICT."""
     f0 = np.asarray(f0, np.float64)
     f1 = np.asarray(f1, np.float64)
     lag_end = len(x) - L + 1 if lag_end is None else lag_end
     if oracle_result is None:
-        rho_o, arg_o = oracle.correlate(x, fs, L, f0, f1, lag_begin, lag_end)
+        rho_o, arg_o = oracle.correlate(x, fs, L, f0, f1, lag_begin, lag_end, f2=f2)
     else:
         rho_o, arg_o = oracle_result
     rho_gpu = np.asarray(rho_gpu, np.float64)
@@ -37,7 +37,8 @@ def check_values_and_argmax(x, fs, L, f0, f1, rho_gpu, arg_gpu, lag_begin=0, lag
     assert np.all((arg_gpu >= lag_begin) & ((arg_gpu < lag_end) | (lag_end == lag_begin)))
     exempt = np.zeros(len(f0), bool)
     for j in np.nonzero(arg_gpu != arg_o)[0]:
-        series = oracle.rho_series(x, fs, L, f0[j], f1[j], lag_begin, lag_end)
+        series = oracle.rho_series(x, fs, L, f0[j], f1[j], lag_begin, lag_end,
+                                   f2=0.0 if f2 is None else float(f2[j]))
         r1 = series[arg_o[j] - lag_begin]
         others = np.delete(series, arg_o[j] - lag_begin)
         r2 = others.max() if len(others) else -np.inf
