@@ -165,7 +165,10 @@ int bfly_make_bank3(double fs_hz, int32_t L, int64_t n_templates, const double *
     BANK_TRY(cudaMalloc((void **)&b->cnt_stage, 2 * sizeof(unsigned long long)));
     BANK_TRY(cudaMemcpy(b->f0, f0_hz, T * sizeof(double), cudaMemcpyHostToDevice));
     BANK_TRY(cudaMemcpy(b->f1, f1_hzps, T * sizeof(double), cudaMemcpyHostToDevice));
-    if (f2_hzps2) { BANK_TRY(cudaMemcpy(b->f2, f2_hzps2, T * sizeof(double), cudaMemcpyHostToDevice)); }
+    if (f2_hzps2) {
+        BANK_TRY(cudaMemcpy(b->f2, f2_hzps2, T * sizeof(double), cudaMemcpyHostToDevice));
+        for (int64_t j = 0; j < n_templates && !b->has_f2; ++j) b->has_f2 = f2_hzps2[j] != 0.0;
+    }
     else { BANK_TRY(cudaMemset(b->f2, 0, T * sizeof(double))); }
 #undef BANK_TRY
     rc = launch_bank_params(b, 0);

@@ -281,7 +281,7 @@ struct TailArgs {
     unsigned long long *n_hits;
 };
 
-template <bool TAILS>
+template <bool TAILS, bool CUBIC>
 __global__ void __launch_bounds__(NT, 1)
 tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const uint64_t *__restrict__ phB, const uint64_t *__restrict__ phC,
@@ -340,7 +340,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         // ---- A3: synthesise g[n] = cos phi_n - i r sin phi_n, r = ||cos phi|| / ||sin phi||,
         //      n = 1024 a + 128 g + 16 c + d' < L, as the operand fragments of pass A (so that
         //      |z|^2 / ||cos phi||^2 is the quadrature sum); direct sums for the tail lags
-        const uint64_t A = phA[j], Bq = phB[j], Cq = phC[j];
+        const uint64_t A = phA[j], Bq = phB[j], Cq = CUBIC ? phC[j] : 0ull;
         const uint32_t Ahi = (uint32_t)(A >> 32), Alo = (uint32_t)A;
         const uint32_t Bhi = (uint32_t)(Bq >> 32), Blo = (uint32_t)Bq;
         const float ic = inc2[j], rq = sqrtf(ins2[j] / ic);   // ic > 0: cos phi_0 = 1
@@ -358,7 +358,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const int n = 1024 * (2 * t + e) + 128 * g + 16 * c + dp;
                     cs[e] = sn[e] = 0.0f;
                     if (n < L) {
-                        if (Cq == 0ull) {            // linear chirp (uniform over the CTA)
+                        if (!CUBIC) {                // linear chirp
                             synth_sincos(Ahi, Alo, Bhi, Blo, (uint32_t)n, &sn[e], &cs[e]);
                         } else {                     // reading N1: cubic phase, full 64-bit Horner
                             const uint32_t ph = (uint32_t)(template_phase(A, Bq, Cq, (uint64_t)n) >> 32);
@@ -661,8 +661,10 @@ static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_sample
     if (!attr_set) {
         BFLY_CUDA(cudaFuncSetAttribute(tc_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_wspec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         attr_set = true;
     }
     const int64_t n_lags = lag_end - lag_begin;
@@ -686,16 +688,19 @@ static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_sample
     }
     const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
     core_timer_start(b, stream);
-    if (tails)
-        tc_correlate_kernel<true><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
-            b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
-            reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
-            rho_max, arg_lag, *tails);
-    else
-        tc_correlate_kernel<false><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(
-            b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),
-            reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,
-            rho_max, arg_lag, TailArgs{});
+#define BFLY_TC_LAUNCH(TAILS_, CUBIC_, ARGS_)                                                          \
+    tc_correlate_kernel<TAILS_, CUBIC_><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(                      \
+        b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh), \
+        reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,    \
+        rho_max, arg_lag, ARGS_)
+    if (tails) {
+        if (b->has_f2) BFLY_TC_LAUNCH(true, true, *tails);
+        else BFLY_TC_LAUNCH(true, false, *tails);
+    } else {
+        if (b->has_f2) BFLY_TC_LAUNCH(false, true, TailArgs{});
+        else BFLY_TC_LAUNCH(false, false, TailArgs{});
+    }
+#undef BFLY_TC_LAUNCH
     core_timer_stop(b, stream);
     count_launch();
     BFLY_CUDA(cudaGetLastError());

@@ -20,6 +20,7 @@ struct bfly_bank {
     uint64_t *phA;   // f0/fs            in units of 2^-64 cycles per sample
     uint64_t *phB;   // f1/(2 fs^2)      in units of 2^-64 cycles per sample^2
     uint64_t *phC;   // f2/(6 fs^3)      in units of 2^-64 cycles per sample^3
+    int has_f2;      // some template has f2 != 0 (selects the cubic-phase kernel variants)
     float *inc2;     // 1 / ||cos phi||^2 (0 if the norm is 0)
     float *ins2;     // 1 / ||sin phi||^2
     // workspace (grown by bfly_bank_reserve / on demand)
