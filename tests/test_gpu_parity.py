@@ -311,3 +311,66 @@ def test_full_bank_config4_sampled_against_the_oracle(bfly):
     np.testing.assert_array_equal(m.cpu().numpy().view(np.uint32), want)
     assert c.cpu().numpy().tolist() == [int(hit.sum()), int((~ok).sum())]
     assert np.all((arg_n >= 0) & (arg_n < cfg.n_lags)) and np.all(np.isfinite(rho_n)) and rho_n.max() < 1.0
+
+
+# ----------------------------------------------------------------- configs 3 and 5 at full size
+def test_full_bank_config3_sampled_against_the_oracle(bfly):
+    """BASELINE.json config 3 at full size (2^20 templates of L = 2000 against 128000 samples:
+    L not a power of two, 31 overlap-save blocks + a ragged last block), sampled templates
+    against the oracle (R1, R2) and bit-identical to a sub-bank run (R4)."""
+    cfg = get_config(3)
+    x = make_data(cfg)
+    xd = torch.from_numpy(x).cuda()
+    full = bfly.make_bank_grid(cfg.fs_hz, cfg.L, cfg.f0_lo, cfg.f0_hi, cfg.n_f0,
+                               cfg.f1_lo, cfg.f1_hi, cfg.n_f1)
+    assert len(full) == 1 << 20
+    rho, arg = bfly.correlate(full, xd)
+    f0a, f1a = bank_grid(cfg)
+    idx = np.unique(np.concatenate([sub_bank_indices(cfg, 28, seed=5),
+                                    [0, cfg.n_f1 - 1, len(f0a) - cfg.n_f1, len(f0a) - 1]]))
+    it = torch.from_numpy(idx).cuda()
+    rho_s, arg_s = rho[it].cpu().numpy(), arg[it].cpu().numpy()
+    check_values_and_argmax(x, cfg.fs_hz, cfg.L, f0a[idx], f1a[idx], rho_s, arg_s)
+    sub = bfly.make_bank(cfg.fs_hz, cfg.L, f0a[idx], f1a[idx])
+    r2, a2 = bfly.correlate(sub, xd)
+    assert np.array_equal(r2.cpu().numpy(), rho_s) and np.array_equal(a2.cpu().numpy(), arg_s)
+
+
+def test_streaming_config5_at_full_size(bfly):
+    """BASELINE.json config 5 at full size: 1024 s (4 194 304 samples) in 16-s chunks with 1-s
+    overlap against 2^20 templates through bfly_search_host (69 chunks), the map accumulated
+    over the whole run.  The map equals, cell by cell, the histogram of the per-chunk outputs of
+    bfly_correlate over the chunk plan of reading C11 (integer, exact); two chunks -- the one
+    holding the injected chirp's start and the ragged tail chunk -- are checked on sampled
+    templates against the oracle (R1, R2)."""
+    cfg = get_config(5)
+    x = make_data(cfg)
+    L, chunk = cfg.L, cfg.chunk_samples
+    bank = bfly.make_bank_grid(cfg.fs_hz, L, cfg.f0_lo, cfg.f0_hi, cfg.n_f0,
+                               cfg.f1_lo, cfg.f1_hi, cfg.n_f1)
+    grid = default_map_grid(cfg)
+    rho_h, arg_h, m_h, cnt_h = bfly.search_host(bank, x, chunk, cfg.kappa, **grid)
+    plan = streaming.chunk_plan(len(x), L, chunk)
+    assert len(plan) == 69 and plan[-1][3] - plan[-1][2] == 12289
+    f0a, f1a = bank_grid(cfg)
+    idx = np.unique(np.concatenate([sub_bank_indices(cfg, 12, seed=9, max_track=6), [0, len(f0a) - 1]]))
+    it = torch.from_numpy(idx).cuda()
+    xd = torch.from_numpy(x).cuda()
+    fb = np.floor((f0a - grid["f_lo_hz"]) / grid["df_hz"]).astype(np.int64)
+    want = np.zeros((grid["n_tbins"], grid["n_fbins"]), np.uint32)
+    hits = dropped = 0
+    chirp_chunk = int(300 * cfg.fs_hz) // (chunk - L)
+    for ci, (s, n, lb, le) in enumerate(plan):
+        rho, arg = bfly.correlate(bank, xd[s:s + n], lb, le)
+        rn, an = rho.cpu().numpy(), arg.cpu().numpy()
+        hit = rn > np.float32(cfg.kappa)
+        tb = (s + an[hit].astype(np.int64)) // grid["samples_per_tbin"]
+        ok = (tb < grid["n_tbins"]) & (fb[hit] >= 0) & (fb[hit] < grid["n_fbins"])
+        np.add.at(want, (tb[ok], fb[hit][ok]), 1)
+        hits += int(hit.sum()); dropped += int((~ok).sum())
+        if ci in (chirp_chunk, len(plan) - 1):
+            check_values_and_argmax(x[s:s + n], cfg.fs_hz, L, f0a[idx], f1a[idx], rn[idx], an[idx], lb, le)
+        if ci == len(plan) - 1:
+            assert np.array_equal(rn, rho_h) and np.array_equal(an, arg_h)
+    np.testing.assert_array_equal(m_h, want)
+    assert cnt_h.tolist() == [hits, dropped]
