@@ -374,3 +374,21 @@ def test_streaming_config5_at_full_size(bfly):
             assert np.array_equal(rn, rho_h) and np.array_equal(an, arg_h)
     np.testing.assert_array_equal(m_h, want)
     assert cnt_h.tolist() == [hits, dropped]
+
+
+@pytest.mark.parametrize("form", [pytest.param(3, id="fft_tc"), pytest.param(4, id="dense_tc"), pytest.param(1, id="fft")])
+def test_one_long_segment_in_a_single_call(bfly, form):
+    """A 600 000-sample segment in ONE call (146 overlap-save blocks, 2328 lag tiles of the dense
+    form; no chunking), five templates: lag indices far beyond one block, workspace growth."""
+    rng = np.random.default_rng(77)
+    fs, L, N = 4096.0, 4096, 600_000
+    x = rng.standard_normal(N)
+    f0 = np.array([150.0, 800.0, 1999.0, 33.3, 1200.0])
+    f1 = np.array([300.0, -120.0, -999.0, 0.7, 45.0])
+    hc, _ = oracle.template(fs, L, f0[1], f1[1])
+    x[555_555:555_555 + L] += 0.4 * hc                       # found near the end of the segment
+    x = x.astype(np.float32)
+    _, rho, arg = _run(bfly, form, fs, L, f0, f1, x)
+    rho_n, arg_n = rho.cpu().numpy(), arg.cpu().numpy()
+    _, arg_o, _ = check_values_and_argmax(x, fs, L, f0, f1, rho_n, arg_n)
+    assert arg_n[1] == arg_o[1] and abs(int(arg_n[1]) - 555_555) <= 4 and rho_n[1] > 0.2
