@@ -56,6 +56,24 @@ def lib():
         L.bfo_tails.argtypes = [fp, C.c_int64, C.c_double, C.c_int, C.c_int64, dp, dp, C.c_int64,
                                 C.c_int64, C.c_double, dp, C.c_int64, ip, ip, dp, C.c_int]
         L.bfo_tails.restype = C.c_int64
+        L.bfo_template_settle.argtypes = [C.c_double, C.c_int, C.c_double, C.c_double, C.c_double, dp, dp]
+        L.bfo_template_settle.restype = None
+        L.bfo_template_family.argtypes = [C.c_int, C.c_double, C.c_int, C.c_double, C.c_double,
+                                          C.c_double, dp, dp]
+        L.bfo_template_family.restype = None
+        L.bfo_rho_series_family.argtypes = [C.c_int, fp, C.c_int64, C.c_double, C.c_int, C.c_double,
+                                            C.c_double, C.c_double, C.c_int64, C.c_int64, dp, dp, dp]
+        L.bfo_rho_series_family.restype = None
+        L.bfo_correlate_family.argtypes = [C.c_int, fp, C.c_int64, C.c_double, C.c_int, C.c_int64,
+                                           dp, dp, dp, C.c_int64, C.c_int64, dp, ip, C.c_int]
+        L.bfo_correlate_family.restype = C.c_int
+        L.bfo_sigma_family.argtypes = [C.c_int, fp, C.c_int64, C.c_double, C.c_int, C.c_double,
+                                       C.c_double, C.c_double]
+        L.bfo_sigma_family.restype = C.c_double
+        L.bfo_tails_family.argtypes = [C.c_int, fp, C.c_int64, C.c_double, C.c_int, C.c_int64, dp,
+                                       dp, dp, C.c_int64, C.c_int64, C.c_double, dp, C.c_int64, ip,
+                                       ip, dp, C.c_int]
+        L.bfo_tails_family.restype = C.c_int64
         L.bfo_max_threads.argtypes = []
         L.bfo_max_threads.restype = C.c_int
         _lib = L
@@ -81,12 +99,22 @@ def max_threads() -> int:
     return int(lib().bfo_max_threads())
 
 
-def template(fs, L, f0, f1, f2=0.0):
-    """(hc, hs): un-normalised cosine and sine templates, float64[L] each (f2: reading N1)."""
+FAMILY = {"poly": 0, "settle": 1}
+
+
+def _fam(family) -> int:
+    """Template family: "poly" = (f0, f1, f2) polynomial phase (readings C1, N1), "settle" =
+    (f_inf, D, tc) exponentially settling chirp (reading N2)."""
+    return FAMILY[family]
+
+
+def template(fs, L, f0, f1, f2=0.0, family="poly"):
+    """(hc, hs): un-normalised cosine and sine templates, float64[L] each.  family "poly":
+    (f0, f1, f2) (f2: reading N1); family "settle": the three arguments are (f_inf, D, tc)."""
     hc = np.empty(L, np.float64)
     hs = np.empty(L, np.float64)
-    lib().bfo_template3(float(fs), int(L), float(f0), float(f1), float(f2), _p(hc, C.c_double),
-                        _p(hs, C.c_double))
+    lib().bfo_template_family(_fam(family), float(fs), int(L), float(f0), float(f1), float(f2),
+                              _p(hc, C.c_double), _p(hs, C.c_double))
     return hc, hs
 
 
@@ -118,7 +146,8 @@ def sliding_n2(x, L, lag_begin=0, lag_end=None):
     return out
 
 
-def rho_series(x, fs, L, f0, f1, lag_begin=0, lag_end=None, components=False, f2=0.0):
+def rho_series(x, fs, L, f0, f1, lag_begin=0, lag_end=None, components=False, f2=0.0,
+               family="poly"):
     """rho(tau) of one template over lag_begin <= tau < lag_end (float64)."""
     x = _f32(x)
     lag_end = len(x) - L + 1 if lag_end is None else lag_end
@@ -132,13 +161,15 @@ def rho_series(x, fs, L, f0, f1, lag_begin=0, lag_end=None, components=False, f2
         cp, sp = _p(c, C.c_double), _p(s, C.c_double)
     else:
         cp = sp = None
-    lib().bfo_rho_series3(_p(x, C.c_float), len(x), float(fs), int(L), float(f0), float(f1),
-                          float(f2), int(lag_begin), int(lag_end), _p(rho, C.c_double), cp, sp)
+    lib().bfo_rho_series_family(_fam(family), _p(x, C.c_float), len(x), float(fs), int(L),
+                                float(f0), float(f1), float(f2), int(lag_begin), int(lag_end),
+                                _p(rho, C.c_double), cp, sp)
     return (rho, c, s) if components else rho
 
 
-def correlate(x, fs, L, f0, f1, lag_begin=0, lag_end=None, n_threads=0, f2=None):
-    """(rho_max float64[T], arg_lag int32[T]) over lag_begin <= tau < lag_end."""
+def correlate(x, fs, L, f0, f1, lag_begin=0, lag_end=None, n_threads=0, f2=None, family="poly"):
+    """(rho_max float64[T], arg_lag int32[T]) over lag_begin <= tau < lag_end.  family "settle":
+    (f0, f1, f2) carry (f_inf, D, tc) per template."""
     x = _f32(x)
     f0, f1 = _f64(f0), _f64(f1)
     if f0.shape != f1.shape or f0.ndim != 1:
@@ -151,11 +182,13 @@ def correlate(x, fs, L, f0, f1, lag_begin=0, lag_end=None, n_threads=0, f2=None)
         f2 = _f64(f2)
         if f2.shape != f0.shape:
             raise ValueError("f2 must have the shape of f0")
-    rc = lib().bfo_correlate3(_p(x, C.c_float), len(x), float(fs), int(L), T,
-                              _p(f0, C.c_double), _p(f1, C.c_double),
-                              _p(f2, C.c_double) if f2 is not None else None, int(lag_begin),
-                              int(lag_end), _p(rho_max, C.c_double), _p(arg, C.c_int32),
-                              int(n_threads))
+    if family == "settle" and f2 is None:
+        raise ValueError("the settle family needs tc per template")
+    rc = lib().bfo_correlate_family(_fam(family), _p(x, C.c_float), len(x), float(fs), int(L), T,
+                                    _p(f0, C.c_double), _p(f1, C.c_double),
+                                    _p(f2, C.c_double) if f2 is not None else None, int(lag_begin),
+                                    int(lag_end), _p(rho_max, C.c_double), _p(arg, C.c_int32),
+                                    int(n_threads))
     if rc < 0:
         raise ValueError("bfo_correlate: bad arguments")
     return rho_max, arg
@@ -178,39 +211,51 @@ def butterfly_map(f0, rho_max, arg_lag, kappa, lag_origin, samples_per_tbin, f_l
     return map_out, counters
 
 
-def sigma(x, fs, L, f0, f1):
+def sigma(x, fs, L, f0, f1, f2=0.0, family="poly"):
     """Reading S1: rms per quadrature of the circular matched-filter output of one template
     over the whole segment."""
     x = _f32(x)
     if len(x) < L:
         raise ValueError("segment shorter than the template")
-    return float(lib().bfo_sigma(_p(x, C.c_float), len(x), float(fs), int(L), float(f0), float(f1)))
+    return float(lib().bfo_sigma_family(_fam(family), _p(x, C.c_float), len(x), float(fs), int(L),
+                                        float(f0), float(f1), float(f2)))
 
 
-def tails(x, fs, L, f0, f1, kappa, lag_begin=0, lag_end=None, capacity=None, n_threads=0):
+def tails(x, fs, L, f0, f1, kappa, lag_begin=0, lag_end=None, capacity=None, n_threads=0,
+          f2=None, family="poly"):
     """Readings S1-S3: (sigma float64[T], hit_template int32[n], hit_lag int32[n],
     hit_rho float64[n], total) with hits = valid lags where sqrt(c^2+s^2)/sigma_j > kappa, in
     ascending (template, lag) order; n = min(total, capacity)."""
     x = _f32(x)
     f0, f1 = _f64(f0), _f64(f1)
+    if f2 is not None:
+        f2 = _f64(f2)
+        if f2.shape != f0.shape:
+            raise ValueError("f2 must have the shape of f0")
+    elif family == "settle":
+        raise ValueError("the settle family needs tc per template")
+    p2 = _p(f2, C.c_double) if f2 is not None else None
+    fam = _fam(family)
     lag_end = len(x) - L + 1 if lag_end is None else lag_end
     T = len(f0)
     sig = np.empty(T, np.float64)
     if capacity is None:
         # count first, then size the arrays exactly
-        total = lib().bfo_tails(_p(x, C.c_float), len(x), float(fs), int(L), T, _p(f0, C.c_double),
-                                _p(f1, C.c_double), int(lag_begin), int(lag_end), float(kappa),
-                                _p(sig, C.c_double), 0, None, None, None, int(n_threads))
+        total = lib().bfo_tails_family(fam, _p(x, C.c_float), len(x), float(fs), int(L), T,
+                                       _p(f0, C.c_double), _p(f1, C.c_double), p2, int(lag_begin),
+                                       int(lag_end), float(kappa), _p(sig, C.c_double), 0, None,
+                                       None, None, int(n_threads))
         if total < 0:
             raise ValueError("bad arguments")
         capacity = int(total)
     hj = np.empty(max(capacity, 1), np.int32)
     hl = np.empty(max(capacity, 1), np.int32)
     hr = np.empty(max(capacity, 1), np.float64)
-    total = lib().bfo_tails(_p(x, C.c_float), len(x), float(fs), int(L), T, _p(f0, C.c_double),
-                            _p(f1, C.c_double), int(lag_begin), int(lag_end), float(kappa),
-                            _p(sig, C.c_double), int(capacity), _p(hj, C.c_int32),
-                            _p(hl, C.c_int32), _p(hr, C.c_double), int(n_threads))
+    total = lib().bfo_tails_family(fam, _p(x, C.c_float), len(x), float(fs), int(L), T,
+                                   _p(f0, C.c_double), _p(f1, C.c_double), p2, int(lag_begin),
+                                   int(lag_end), float(kappa), _p(sig, C.c_double), int(capacity),
+                                   _p(hj, C.c_int32), _p(hl, C.c_int32), _p(hr, C.c_double),
+                                   int(n_threads))
     if total < 0:
         raise ValueError("bad arguments")
     n = int(min(total, capacity))

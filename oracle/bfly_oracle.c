@@ -23,7 +23,9 @@
  * P2 noise-free injection, P3 time reversal, P4 direct vs FFT, P5 scale
  * invariance, P6 DFT special case against numpy.fft, P7 Parseval sum, P8 noise
  * expectation 2/L, P9 matched injection in noise, P10 map by brute force,
- * P11 chunking; PS1-PS5 for the kappa-sigma tails (bfo_sigma, bfo_tails).  Parity unpinned (fixed by DESIGN.md readings only, the paper
+ * P11 chunking; PS1-PS6 for the kappa-sigma tails (bfo_sigma*, bfo_tails*); PN1-PN4 for the
+ * cubic-phase family, PE1-PE5 for the exponentially settling family, PD1-PD2 for the phase
+ * reduction (C4).  Parity unpinned (fixed by DESIGN.md readings only, the paper
  * being silent): the choice of map coordinates (C10: time = start of the matched
  * window, frequency = f0) and the per-chunk hit semantics of streaming (C11).
  *
@@ -41,21 +43,40 @@
 
 #define BFO_PI 3.14159265358979323846
 
+/* cos and sin of a phase given in CYCLES (reading C4 of DESIGN.md: the phase is defined modulo one
+ * turn, so it is reduced modulo 1 before the trigonometric call).  frac = cyc - floor(cyc) is
+ * exact in float64; the nearest quarter turn is split off (also exact) so that the values at
+ * multiples of a quarter turn are exactly 0 and +-1 -- the template (f0 = fs/2, f1 = 0) then has a
+ * sine part that is identically zero, as the definition says, rather than rounding noise of
+ * sin(pi k) that a later normalisation would blow up. */
+static void bfo_sincos_cycles(double cyc, double *s, double *c)
+{
+    double frac = cyc - floor(cyc);                  /* in [0, 1) */
+    int q = (int)floor(4.0 * frac + 0.5);            /* nearest quarter turn, 0..4 */
+    double r = frac - 0.25 * (double)q;              /* in [-1/8, 1/8], exact */
+    double s0 = sin(2.0 * BFO_PI * r), c0 = cos(2.0 * BFO_PI * r);
+    switch (q & 3) {
+        case 0: *s = s0;  *c = c0;  break;
+        case 1: *s = c0;  *c = -s0; break;
+        case 2: *s = -s0; *c = -c0; break;
+        default: *s = -c0; *c = s0; break;
+    }
+}
+
 /* C1 (BASELINE.json configs[0]): template samples
  *   t_k = k/fs, phi_k = 2 pi (f0 t_k + 1/2 f1 t_k^2), hc[k] = cos phi_k, hs[k] = sin phi_k,
- *   k = 0..L-1; phase zero at the first sample; no window. */
+ *   k = 0..L-1; phase zero at the first sample; no window.  The bracket is the phase in cycles. */
 void bfo_template(double fs, int L, double f0, double f1, double *hc, double *hs)
 {
     for (int k = 0; k < L; ++k) {
         double t = (double)k / fs;
-        double phi = 2.0 * BFO_PI * (f0 * t + 0.5 * f1 * t * t);
-        hc[k] = cos(phi);
-        hs[k] = sin(phi);
+        double cyc = f0 * t + 0.5 * f1 * t * t;
+        bfo_sincos_cycles(cyc, &hs[k], &hc[k]);
     }
 }
 
 /* N1 (descending chirps that settle
- * towards a late-time plateau; the paper gives no waveform): the non-linear family is the chirp
+ * towards a late-time plateau; the paper gives no waveform): the cubic-phase family is the chirp
  * with a constant second frequency derivative f2 [Hz/s^2],
  *   f(t) = f0 + f1 t + 1/2 f2 t^2,   phi_k = 2 pi (f0 t_k + 1/2 f1 t_k^2 + 1/6 f2 t_k^3),
  * which represents an exponentially settling chirp f_inf + D exp(-t/tc) over one template by its
@@ -65,10 +86,35 @@ void bfo_template3(double fs, int L, double f0, double f1, double f2, double *hc
     if (f2 == 0.0) { bfo_template(fs, L, f0, f1, hc, hs); return; }
     for (int k = 0; k < L; ++k) {
         double t = (double)k / fs;
-        double phi = 2.0 * BFO_PI * (f0 * t + 0.5 * f1 * t * t + f2 * t * t * t / 6.0);
-        hc[k] = cos(phi);
-        hs[k] = sin(phi);
+        double cyc = f0 * t + 0.5 * f1 * t * t + f2 * t * t * t / 6.0;
+        bfo_sincos_cycles(cyc, &hs[k], &hc[k]);
     }
+}
+
+/* N2 (SURVEY.md section 8(f) rank 4 "exponentially settling descending chirps ... synthesised
+ * from 3-4 parameters"; PAPER.md:21-26 (sec. 1, Eq. 1: descending chirps that "reach a late time
+ * plateau" f_GW), PAPER.md:60 (Fig. 2, right)): the settling family itself,
+ *   f(t) = f_inf + D exp(-t / tc),     phi_k = 2 pi ( f_inf t_k + D tc (1 - exp(-t_k / tc)) ),
+ * D = f(0) - f_inf [Hz] (D > 0 descends towards the plateau f_inf), tc > 0 the settling time [s].
+ * 1 - exp(-u) is taken as -expm1(-u), which keeps full precision for t << tc. */
+void bfo_template_settle(double fs, int L, double f_inf, double D, double tc, double *hc, double *hs)
+{
+    for (int k = 0; k < L; ++k) {
+        double t = (double)k / fs;
+        double cyc = f_inf * t + D * tc * (-expm1(-t / tc));
+        bfo_sincos_cycles(cyc, &hs[k], &hc[k]);
+    }
+}
+
+/* One entry for both families: family 0 = (f0, f1, f2) polynomial phase (C1 / N1),
+ * family 1 = (f_inf, D, tc) exponentially settling (N2). */
+#define BFO_FAMILY_POLY 0
+#define BFO_FAMILY_SETTLE 1
+void bfo_template_family(int family, double fs, int L, double p0, double p1, double p2, double *hc,
+                         double *hs)
+{
+    if (family == BFO_FAMILY_SETTLE) bfo_template_settle(fs, L, p0, p1, p2, hc, hs);
+    else bfo_template3(fs, L, p0, p1, p2, hc, hs);
 }
 
 /* C2 ("each unit-L2-normalized", BASELINE.json configs[0]): the L2 norms of the
@@ -160,26 +206,33 @@ static void bfo_dots_run(const double *restrict xd, int L, const double *restric
 
 /* rho_j(tau) of ONE template for lag_begin <= tau < lag_end (needed for the argmax
  * rule and the pins).  c_out / s_out (optional) receive c/||x_tau||, s/||x_tau||. */
+void bfo_rho_series_family(int family, const float *x, int64_t n_samples, double fs, int L,
+                           double p0, double p1, double p2, int64_t lag_begin, int64_t lag_end,
+                           double *rho, double *c_out, double *s_out);
 void bfo_rho_series3(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
                      double f2, int64_t lag_begin, int64_t lag_end, double *rho, double *c_out,
-                     double *s_out);
+                     double *s_out)
+{
+    bfo_rho_series_family(BFO_FAMILY_POLY, x, n_samples, fs, L, f0, f1, f2, lag_begin, lag_end, rho,
+                          c_out, s_out);
+}
 void bfo_rho_series(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
                     int64_t lag_begin, int64_t lag_end, double *rho, double *c_out, double *s_out)
 {
     bfo_rho_series3(x, n_samples, fs, L, f0, f1, 0.0, lag_begin, lag_end, rho, c_out, s_out);
 }
 
-/* The same for a template of the non-linear family (N1). */
-void bfo_rho_series3(const float *x, int64_t n_samples, double fs, int L, double f0, double f1,
-                     double f2, int64_t lag_begin, int64_t lag_end, double *rho, double *c_out,
-                     double *s_out)
+/* The same for a template of either family (N1: p = (f0, f1, f2); N2: p = (f_inf, D, tc)). */
+void bfo_rho_series_family(int family, const float *x, int64_t n_samples, double fs, int L,
+                           double p0, double p1, double p2, int64_t lag_begin, int64_t lag_end,
+                           double *rho, double *c_out, double *s_out)
 {
     double *xd = (double *)malloc(sizeof(double) * (size_t)n_samples);
     for (int64_t i = 0; i < n_samples; ++i) xd[i] = (double)x[i];
     double *hc = (double *)malloc(sizeof(double) * (size_t)L);
     double *hs = (double *)malloc(sizeof(double) * (size_t)L);
     double nc, ns;
-    bfo_template3(fs, L, f0, f1, f2, hc, hs);
+    bfo_template_family(family, fs, L, p0, p1, p2, hc, hs);
     bfo_template_norms(L, hc, hs, &nc, &ns);
     double c[BFO_RUN], s[BFO_RUN];
     for (int64_t tau0 = lag_begin; tau0 < lag_end; tau0 += BFO_RUN) {
@@ -211,9 +264,17 @@ void bfo_rho_series3(const float *x, int64_t n_samples, double fs, int L, double
  * lags only (C5): requires 0 <= lag_begin <= lag_end <= n_samples - L + 1.
  * Templates are independent; OpenMP runs them on n_threads threads (0 = default).
  * Returns the number of threads used, or -1 on bad arguments. */
+int bfo_correlate_family(int family, const float *x, int64_t n_samples, double fs, int L,
+                         int64_t n_templates, const double *p0, const double *p1, const double *p2,
+                         int64_t lag_begin, int64_t lag_end, double *rho_max, int32_t *arg_lag,
+                         int n_threads);
 int bfo_correlate3(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
                    const double *f0, const double *f1, const double *f2, int64_t lag_begin,
-                   int64_t lag_end, double *rho_max, int32_t *arg_lag, int n_threads);
+                   int64_t lag_end, double *rho_max, int32_t *arg_lag, int n_threads)
+{
+    return bfo_correlate_family(BFO_FAMILY_POLY, x, n_samples, fs, L, n_templates, f0, f1, f2,
+                                lag_begin, lag_end, rho_max, arg_lag, n_threads);
+}
 int bfo_correlate(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
                   const double *f0, const double *f1, int64_t lag_begin, int64_t lag_end,
                   double *rho_max, int32_t *arg_lag, int n_threads)
@@ -222,10 +283,12 @@ int bfo_correlate(const float *x, int64_t n_samples, double fs, int L, int64_t n
                           arg_lag, n_threads);
 }
 
-/* The same with a per-template second frequency derivative f2 (N1); f2 == NULL means 0. */
-int bfo_correlate3(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
-                   const double *f0, const double *f1, const double *f2, int64_t lag_begin,
-                   int64_t lag_end, double *rho_max, int32_t *arg_lag, int n_threads)
+/* The same for either family: per-template parameters (p0, p1, p2) = (f0, f1, f2) (N1) or
+ * (f_inf, D, tc) (N2); p2 == NULL means 0 (polynomial family only). */
+int bfo_correlate_family(int family, const float *x, int64_t n_samples, double fs, int L,
+                         int64_t n_templates, const double *p0, const double *p1, const double *p2,
+                         int64_t lag_begin, int64_t lag_end, double *rho_max, int32_t *arg_lag,
+                         int n_threads)
 {
     if (L < 1 || n_samples < L || lag_begin < 0 || lag_end < lag_begin ||
         lag_end > n_samples - L + 1)
@@ -250,7 +313,7 @@ int bfo_correlate3(const float *x, int64_t n_samples, double fs, int L, int64_t 
 #pragma omp for schedule(dynamic, 1)
         for (int64_t j = 0; j < n_templates; ++j) {
             double nc, ns;
-            bfo_template3(fs, L, f0[j], f1[j], f2 ? f2[j] : 0.0, hc, hs);
+            bfo_template_family(family, fs, L, p0[j], p1[j], p2 ? p2[j] : 0.0, hc, hs);
             bfo_template_norms(L, hc, hs, &nc, &ns);
             double best = -1.0;
             int64_t arg = lag_begin;
@@ -314,15 +377,18 @@ void bfo_map(int64_t n_templates, const double *f0, const double *rho_max, const
  *         rho_sigma(tau) = sqrt(c(tau)^2 + s(tau)^2) / sigma  >  kappa      (strict, C9),
  *     with c, s the unit-norm-template sums of bfo_rho_at (not divided by ||x_tau||).
  * S3  sigma == 0 (all-zero segment): no hits.
+ * The tails apply to whatever bank is searched, so every function below takes
+ * the template family; bfo_sigma / bfo_tails are the linear-chirp entry points.
  * ------------------------------------------------------------------------------------- */
 
-/* S1, written out in the time domain (N L multiply-adds). */
-double bfo_sigma(const float *x, int64_t n_samples, double fs, int L, double f0, double f1)
+/* S1, written out in the time domain (N L multiply-adds), for a template of either family. */
+double bfo_sigma_family(int family, const float *x, int64_t n_samples, double fs, int L, double p0,
+                        double p1, double p2)
 {
     double *hc = (double *)malloc(sizeof(double) * (size_t)L);
     double *hs = (double *)malloc(sizeof(double) * (size_t)L);
     double nc, ns, acc = 0.0;
-    bfo_template(fs, L, f0, f1, hc, hs);
+    bfo_template_family(family, fs, L, p0, p1, p2, hc, hs);
     bfo_template_norms(L, hc, hs, &nc, &ns);
     for (int64_t tau = 0; tau < n_samples; ++tau) {
         double c = 0.0, s = 0.0;
@@ -340,14 +406,19 @@ double bfo_sigma(const float *x, int64_t n_samples, double fs, int L, double f0,
     free(hc); free(hs);
     return sqrt(acc / (2.0 * (double)n_samples));
 }
+double bfo_sigma(const float *x, int64_t n_samples, double fs, int L, double f0, double f1)
+{
+    return bfo_sigma_family(BFO_FAMILY_POLY, x, n_samples, fs, L, f0, f1, 0.0);
+}
 
 /* S1-S3 for a list of templates.  sigma[j] is always written.  Hits are stored in ascending
  * (template, lag) order, the first `capacity` of them; the return value is the total number
  * of hits (which may exceed capacity), or -1 on bad arguments. */
-int64_t bfo_tails(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
-                  const double *f0, const double *f1, int64_t lag_begin, int64_t lag_end,
-                  double kappa, double *sigma, int64_t capacity, int32_t *hit_template,
-                  int32_t *hit_lag, double *hit_rho, int n_threads)
+int64_t bfo_tails_family(int family, const float *x, int64_t n_samples, double fs, int L,
+                         int64_t n_templates, const double *p0, const double *p1, const double *p2,
+                         int64_t lag_begin, int64_t lag_end, double kappa, double *sigma,
+                         int64_t capacity, int32_t *hit_template, int32_t *hit_lag, double *hit_rho,
+                         int n_threads)
 {
     if (L < 1 || n_samples < L || lag_begin < 0 || lag_end < lag_begin ||
         lag_end > n_samples - L + 1)
@@ -363,7 +434,7 @@ int64_t bfo_tails(const float *x, int64_t n_samples, double fs, int L, int64_t n
     /* pass 1: sigma and the number of hits of every template */
 #pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads)
     for (int64_t j = 0; j < n_templates; ++j)
-        sigma[j] = bfo_sigma(x, n_samples, fs, L, f0[j], f1[j]);
+        sigma[j] = bfo_sigma_family(family, x, n_samples, fs, L, p0[j], p1[j], p2 ? p2[j] : 0.0);
     int64_t total = 0;
     for (int pass = 0; pass < 2; ++pass) {
         /* pass 0 counts, pass 1 stores at the offsets the counts give (ascending order) */
@@ -379,7 +450,7 @@ int64_t bfo_tails(const float *x, int64_t n_samples, double fs, int L, int64_t n
 #pragma omp for schedule(dynamic, 1)
             for (int64_t j = 0; j < n_templates; ++j) {
                 double nc, ns;
-                bfo_template(fs, L, f0[j], f1[j], hc, hs);
+                bfo_template_family(family, fs, L, p0[j], p1[j], p2 ? p2[j] : 0.0, hc, hs);
                 bfo_template_norms(L, hc, hs, &nc, &ns);
                 int64_t n_hit = 0;
                 for (int64_t tau0 = lag_begin; tau0 < lag_end && sigma[j] > 0.0; tau0 += BFO_RUN) {
@@ -410,6 +481,14 @@ int64_t bfo_tails(const float *x, int64_t n_samples, double fs, int L, int64_t n
     }
     free(count); free(xd);
     return total;
+}
+int64_t bfo_tails(const float *x, int64_t n_samples, double fs, int L, int64_t n_templates,
+                  const double *f0, const double *f1, int64_t lag_begin, int64_t lag_end,
+                  double kappa, double *sigma, int64_t capacity, int32_t *hit_template,
+                  int32_t *hit_lag, double *hit_rho, int n_threads)
+{
+    return bfo_tails_family(BFO_FAMILY_POLY, x, n_samples, fs, L, n_templates, f0, f1, 0, lag_begin,
+                            lag_end, kappa, sigma, capacity, hit_template, hit_lag, hit_rho, n_threads);
 }
 
 int bfo_max_threads(void)

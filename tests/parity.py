@@ -17,14 +17,14 @@ KAPPA_BAND = 2e-4    # R3
 
 
 def check_values_and_argmax(x, fs, L, f0, f1, rho_gpu, arg_gpu, lag_begin=0, lag_end=None,
-                            oracle_result=None, f2=None):
+                            oracle_result=None, f2=None, family="poly"):
     """R1, R2a, R2b for every template.  Returns (rho_oracle, arg_oracle, exempt) where
     exempt[j] is True when template j's argmax is not unique to within GAP_STRICT."""
     f0 = np.asarray(f0, np.float64)
     f1 = np.asarray(f1, np.float64)
     lag_end = len(x) - L + 1 if lag_end is None else lag_end
     if oracle_result is None:
-        rho_o, arg_o = oracle.correlate(x, fs, L, f0, f1, lag_begin, lag_end, f2=f2)
+        rho_o, arg_o = oracle.correlate(x, fs, L, f0, f1, lag_begin, lag_end, f2=f2, family=family)
     else:
         rho_o, arg_o = oracle_result
     rho_gpu = np.asarray(rho_gpu, np.float64)
@@ -38,7 +38,7 @@ def check_values_and_argmax(x, fs, L, f0, f1, rho_gpu, arg_gpu, lag_begin=0, lag
     exempt = np.zeros(len(f0), bool)
     for j in np.nonzero(arg_gpu != arg_o)[0]:
         series = oracle.rho_series(x, fs, L, f0[j], f1[j], lag_begin, lag_end,
-                                   f2=0.0 if f2 is None else float(f2[j]))
+                                   f2=0.0 if f2 is None else float(f2[j]), family=family)
         r1 = series[arg_o[j] - lag_begin]
         others = np.delete(series, arg_o[j] - lag_begin)
         r2 = others.max() if len(others) else -np.inf
@@ -85,7 +85,7 @@ SIGMA_RTOL = 1e-3    # R5: relative tolerance on sigma_j
 
 
 def check_tails(x, fs, L, f0, f1, kappa, sigma_gpu, hit_j, hit_lag, hit_rho, total, lag_begin=0,
-                lag_end=None):
+                lag_end=None, f2=None, family="poly"):
     """R5: the kappa-sigma tails of the CUDA path against oracle.sigma / the oracle's
     series.  rho_sigma = rho ||x_tau|| / sigma, so north_star's |d rho| <= 2e-4 becomes the
     per-hit tolerance tol = 2e-4 ||x_tau|| / sigma_j + SIGMA_RTOL rho_sigma.  (i) sigma within
@@ -95,7 +95,8 @@ def check_tails(x, fs, L, f0, f1, kappa, sigma_gpu, hit_j, hit_lag, hit_rho, tot
     f0 = np.asarray(f0, np.float64)
     f1 = np.asarray(f1, np.float64)
     lag_end = len(x) - L + 1 if lag_end is None else lag_end
-    sig_o = np.array([oracle.sigma(x, fs, L, a, b) for a, b in zip(f0, f1)])
+    f2 = np.zeros(len(f0)) if f2 is None else np.asarray(f2, np.float64)
+    sig_o = np.array([oracle.sigma(x, fs, L, a, b, c, family=family) for a, b, c in zip(f0, f1, f2)])
     sigma_gpu = np.asarray(sigma_gpu, np.float64)
     ok = sig_o > 0
     assert np.all(sigma_gpu[~ok] == 0.0)
@@ -112,7 +113,8 @@ def check_tails(x, fs, L, f0, f1, kappa, sigma_gpu, hit_j, hit_lag, hit_rho, tot
     for j in range(len(f0)):
         if not ok[j]:
             continue
-        rs = oracle.rho_series(x, fs, L, f0[j], f1[j], lag_begin, lag_end) * np.sqrt(n2) / sig_o[j]
+        rs = oracle.rho_series(x, fs, L, f0[j], f1[j], lag_begin, lag_end, f2=float(f2[j]),
+                               family=family) * np.sqrt(n2) / sig_o[j]
         tol = 2e-4 * np.sqrt(n2) / sig_o[j] + SIGMA_RTOL * rs
         mine = {lag for (jj, lag) in got if jj == j}
         for lag in mine:
