@@ -29,6 +29,13 @@
  *    take a stream are asynchronous: they enqueue work and return; kernel faults surface as
  *    BFLY_ECUDA at a later call or at the caller's synchronisation.
  *  - Invalid arguments return BFLY_EINVAL before anything is launched.
+ *  - Every call that takes a bank runs on the bank's device and restores the calling thread's
+ *    current CUDA device before it returns; one process may hold banks on several devices.
+ *  - The workspace inside a bank is one set of buffers.  A call that uses it (bfly_correlate*,
+ *    bfly_tails, bfly_search_host, bfly_bank_reserve) while another thread is inside such a call
+ *    on the same bank returns BFLY_EINVAL ("in use") instead of racing; successive calls on
+ *    different streams are ordered by the library (the later stream waits for the earlier
+ *    call's kernels), so results are as if the calls had been issued on one stream.
  *  - There is no CPU fallback: on a machine without an sm_100 device every call that needs the
  *    GPU returns BFLY_EUNSUPPORTED or BFLY_ECUDA.
  */
@@ -127,7 +134,8 @@ int bfly_bank_reserve(bfly_bank *bank, int64_t max_n_samples);
  * x_dev[0].  An empty lag range gives rho_max = 0, arg_lag = lag_begin.  n_samples < 2^31.
  * Asynchronous on `stream`; no host synchronisation; no allocation if the workspace is
  * already large enough (see bfly_bank_reserve).  One call at a time per bank (the workspace
- * is shared). */
+ * is shared): a concurrent second call from another thread returns BFLY_EINVAL, and a call on
+ * another stream than the previous one is ordered after it (Conventions above). */
 int bfly_correlate(const bfly_bank *bank, const float *x_dev, int64_t n_samples,
                    int64_t lag_begin, int64_t lag_end,
                    float *rho_max_dev, int32_t *arg_lag_dev, void *stream);

@@ -50,10 +50,34 @@ static int select_device(int device, int *sm_count)
                   p.minor);
         return BFLY_EUNSUPPORTED;
     }
-    BFLY_CUDA(cudaSetDevice(device));
     *sm_count = p.multiProcessorCount;
     return BFLY_OK;
 }
+
+// Workspace hand-over between streams: a call on another stream than the previous workspace-using
+// call first waits for that call's work (the workspace is one set of buffers per bank).
+static int ws_begin(bfly_bank *b, cudaStream_t st)
+{
+    if (b->ws_valid && b->ws_stream != st) BFLY_CUDA(cudaStreamWaitEvent(st, b->ws_event, 0));
+    return BFLY_OK;
+}
+static int ws_end(bfly_bank *b, cudaStream_t st)
+{
+    BFLY_CUDA(cudaEventRecord(b->ws_event, st));
+    b->ws_stream = st;
+    b->ws_valid = 1;
+    return BFLY_OK;
+}
+
+#define BFLY_ENTER(bank_)                                                                  \
+    DeviceGuard dev_guard__((bank_)->device);                                              \
+    if (dev_guard__.err != cudaSuccess) return cuda_fail(dev_guard__.err, "cudaSetDevice")
+#define BFLY_LOCK(bank_)                                                                   \
+    BankLock bank_lock__(bank_);                                                           \
+    if (!bank_lock__.held) {                                                               \
+        set_error("the bank is in use by another call (one call at a time per bank)");     \
+        return BFLY_EINVAL;                                                                \
+    }
 
 template <typename T>
 static int grow(T **ptr, int64_t *cap, int64_t need)
@@ -108,13 +132,14 @@ int64_t bfly_launch_count(void) { return g_launches.load(std::memory_order_relax
 void bfly_free_bank(bfly_bank *b)
 {
     if (!b) return;
-    cudaSetDevice(b->device);
+    DeviceGuard guard(b->device);
     cudaFree(b->f0); cudaFree(b->f1); cudaFree(b->f2); cudaFree(b->phA); cudaFree(b->phB); cudaFree(b->phC);
     cudaFree(b->inc2); cudaFree(b->ins2); cudaFree(b->rn2); cudaFree(b->xspec);
     cudaFree(b->xh); cudaFree(b->rn2p); cudaFree(b->qs);
     cudaFree(b->ys); cudaFree(b->rn2s); cudaFree(b->maxbits); cudaFree(b->racf); cudaFree(b->wspec);
     cudaFree(b->packed); cudaFree(b->x_stage); cudaFree(b->rho_stage); cudaFree(b->arg_stage);
     cudaFree(b->map_stage); cudaFree(b->cnt_stage);
+    if (b->ws_event) cudaEventDestroy(b->ws_event);
     if (b->ev_start) cudaEventDestroy(b->ev_start);
     if (b->ev_stop) cudaEventDestroy(b->ev_stop);
     delete b;
@@ -144,6 +169,8 @@ int bfly_make_bank3(double fs_hz, int32_t L, int64_t n_templates, const double *
     int sms = 0;
     int rc = select_device(device, &sms);
     if (rc) return rc;
+    DeviceGuard guard(device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
     bfly_bank *b = new (std::nothrow) bfly_bank();
     if (!b) { set_error("host allocation failed"); return BFLY_ENOMEM; }
     memset(b, 0, sizeof(*b));
@@ -151,6 +178,7 @@ int bfly_make_bank3(double fs_hz, int32_t L, int64_t n_templates, const double *
     const size_t T = (size_t)n_templates;
     cudaError_t e;
 #define BANK_TRY(call) if ((e = (call)) != cudaSuccess) { rc = cuda_fail(e, #call); bfly_free_bank(b); return rc; }
+    BANK_TRY(cudaEventCreateWithFlags(&b->ws_event, cudaEventDisableTiming));
     BANK_TRY(cudaMalloc((void **)&b->f0, T * sizeof(double)));
     BANK_TRY(cudaMalloc((void **)&b->f1, T * sizeof(double)));
     BANK_TRY(cudaMalloc((void **)&b->phA, T * sizeof(uint64_t)));
@@ -211,7 +239,7 @@ int bfly_bank_get(const bfly_bank *b, int64_t first, int64_t count, double *f0_h
 {
     if (!b) { set_error("null bank"); return BFLY_EINVAL; }
     if (first < 0 || count < 0 || first + count > b->T) { set_error("template range outside the bank"); return BFLY_EINVAL; }
-    BFLY_CUDA(cudaSetDevice(b->device));
+    BFLY_ENTER(b);
     const size_t n = (size_t)count;
     if (f0_hz) BFLY_CUDA(cudaMemcpy(f0_hz, b->f0 + first, n * sizeof(double), cudaMemcpyDeviceToHost));
     if (f1_hzps) BFLY_CUDA(cudaMemcpy(f1_hzps, b->f1 + first, n * sizeof(double), cudaMemcpyDeviceToHost));
@@ -224,7 +252,7 @@ int bfly_bank_get_f2(const bfly_bank *b, int64_t first, int64_t count, double *f
 {
     if (!b || !f2_hzps2) { set_error("null pointer"); return BFLY_EINVAL; }
     if (first < 0 || count < 0 || first + count > b->T) { set_error("template range outside the bank"); return BFLY_EINVAL; }
-    BFLY_CUDA(cudaSetDevice(b->device));
+    BFLY_ENTER(b);
     BFLY_CUDA(cudaMemcpy(f2_hzps2, b->f2 + first, (size_t)count * sizeof(double), cudaMemcpyDeviceToHost));
     return BFLY_OK;
 }
@@ -234,14 +262,16 @@ int bfly_bank_reserve(bfly_bank *b, int64_t max_n_samples)
     if (!b) { set_error("null bank"); return BFLY_EINVAL; }
     if (max_n_samples < b->L) { set_error("max_n_samples < L"); return BFLY_EINVAL; }
     if (max_n_samples >= (1LL << 31)) { set_error("segment too long"); return BFLY_ERANGE; }
-    BFLY_CUDA(cudaSetDevice(b->device));
+    BFLY_ENTER(b);
+    BFLY_LOCK(b);
+    if (b->ws_valid) BFLY_CUDA(cudaEventSynchronize(b->ws_event));   // buffers may be freed below
     return reserve_for(b, max_n_samples);
 }
 
 int bfly_bank_set_timing(bfly_bank *b, int enable)
 {
     if (!b) { set_error("null bank"); return BFLY_EINVAL; }
-    BFLY_CUDA(cudaSetDevice(b->device));
+    BFLY_ENTER(b);
     if (enable && !b->ev_start) {
         BFLY_CUDA(cudaEventCreate(&b->ev_start));
         BFLY_CUDA(cudaEventCreate(&b->ev_stop));
@@ -255,15 +285,18 @@ int bfly_bank_core_ms(bfly_bank *b, float *ms_out)
 {
     if (!b || !ms_out) { set_error("null pointer"); return BFLY_EINVAL; }
     if (!b->timing || !b->timed) { set_error("no timed bfly_correlate call on this bank"); return BFLY_EINVAL; }
+    BFLY_ENTER(b);
     BFLY_CUDA(cudaEventSynchronize(b->ev_stop));
     BFLY_CUDA(cudaEventElapsedTime(ms_out, b->ev_start, b->ev_stop));
     return BFLY_OK;
 }
 
-int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int64_t n_samples,
-                        int64_t lag_begin, int64_t lag_end, float *rho_max_dev,
-                        int32_t *arg_lag_dev, void *stream)
+// Argument checks of bfly_correlate_form (before any device work); resolves BFLY_FORM_DEFAULT.
+static int correlate_check(const bfly_bank *bank, int *form_io, const float *x_dev, int64_t n_samples,
+                           int64_t lag_begin, int64_t lag_end, const float *rho_max_dev,
+                           const int32_t *arg_lag_dev)
 {
+    int form = *form_io;
     if (!bank || !x_dev || !rho_max_dev || !arg_lag_dev) { set_error("null pointer"); return BFLY_EINVAL; }
     if (n_samples < bank->L) { set_error("n_samples < L"); return BFLY_EINVAL; }
     if (n_samples >= (1LL << 31)) { set_error("segment too long (n_samples must be < 2^31)"); return BFLY_ERANGE; }
@@ -280,20 +313,44 @@ int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int
         return BFLY_EUNSUPPORTED;
     }
     if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT && form != BFLY_FORM_FFT_TC && form != BFLY_FORM_DENSE_TC) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
+    *form_io = form;
+    return BFLY_OK;
+}
+
+// bfly_correlate_form with the arguments checked, the device selected and the bank locked
+static int correlate_locked(const bfly_bank *bank, int form, const float *x_dev, int64_t n_samples,
+                            int64_t lag_begin, int64_t lag_end, float *rho_max_dev,
+                            int32_t *arg_lag_dev, void *stream)
+{
     bfly_bank *b = const_cast<bfly_bank *>(bank);   // the workspace is mutable state of the bank
-    BFLY_CUDA(cudaSetDevice(b->device));
-    int rc = reserve_for(b, n_samples);
-    if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    int rc = ws_begin(b, st);
+    if (rc) return rc;
+    if ((rc = reserve_for(b, n_samples))) return rc;
     rc = launch_sliding_norm(x_dev, n_samples, b->L, lag_begin, lag_end - lag_begin, b->rn2, st);
     if (rc) return rc;
     if (form == BFLY_FORM_DIRECT)
-        return launch_direct(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
-    if (form == BFLY_FORM_DENSE_TC)
-        return launch_dense_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
-    if (form == BFLY_FORM_FFT)
-        return launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
-    return launch_fft_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+        rc = launch_direct(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    else if (form == BFLY_FORM_DENSE_TC)
+        rc = launch_dense_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    else if (form == BFLY_FORM_FFT)
+        rc = launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    else
+        rc = launch_fft_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    if (rc) return rc;
+    return ws_end(b, st);
+}
+
+int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int64_t n_samples,
+                        int64_t lag_begin, int64_t lag_end, float *rho_max_dev,
+                        int32_t *arg_lag_dev, void *stream)
+{
+    int rc = correlate_check(bank, &form, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev);
+    if (rc) return rc;
+    BFLY_ENTER(bank);
+    BFLY_LOCK(bank);
+    return correlate_locked(bank, form, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev,
+                            stream);
 }
 
 int bfly_tails(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int64_t lag_begin,
@@ -319,16 +376,20 @@ int bfly_tails(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int
         return BFLY_EUNSUPPORTED;
     }
     bfly_bank *b = const_cast<bfly_bank *>(bank);
-    BFLY_CUDA(cudaSetDevice(b->device));
-    int rc = reserve_for(b, n_samples);
+    BFLY_ENTER(b);
+    BFLY_LOCK(b);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ws_begin(b, st);
     if (rc) return rc;
+    if ((rc = reserve_for(b, n_samples))) return rc;
     if (!b->racf) BFLY_CUDA(cudaMalloc((void **)&b->racf, sizeof(double) * FFT_MAX_L));
     if (!b->wspec) BFLY_CUDA(cudaMalloc((void **)&b->wspec, sizeof(float) * FFT_B));
-    cudaStream_t st = (cudaStream_t)stream;
     // rn2 serves the direct tail lags of the kernel's geometry in the other mode; not needed here
-    return launch_tails_tc(b, x_dev, n_samples, lag_begin, lag_end, kappa, sigma_dev, capacity,
-                           hit_template_dev, hit_lag_dev, hit_rho_dev,
-                           (unsigned long long *)n_hits_dev, st);
+    rc = launch_tails_tc(b, x_dev, n_samples, lag_begin, lag_end, kappa, sigma_dev, capacity,
+                         hit_template_dev, hit_lag_dev, hit_rho_dev,
+                         (unsigned long long *)n_hits_dev, st);
+    if (rc) return rc;
+    return ws_end(b, st);
 }
 
 int bfly_hits_map(const bfly_bank *bank, const int32_t *hit_template_dev, const int32_t *hit_lag_dev,
@@ -340,7 +401,7 @@ int bfly_hits_map(const bfly_bank *bank, const int32_t *hit_template_dev, const 
     if (n_hits < 0 || (n_hits > 0 && (!hit_template_dev || !hit_lag_dev))) { set_error("bad hit list"); return BFLY_EINVAL; }
     if (!(df_hz > 0.0) || !std::isfinite(df_hz) || !std::isfinite(f_lo_hz)) { set_error("df must be finite and > 0, f_lo finite"); return BFLY_EINVAL; }
     if (samples_per_tbin <= 0 || n_fbins <= 0 || n_tbins <= 0 || lag_origin < 0) { set_error("bad map geometry"); return BFLY_EINVAL; }
-    BFLY_CUDA(cudaSetDevice(bank->device));
+    BFLY_ENTER(bank);
     return launch_hits_map(bank, hit_template_dev, hit_lag_dev, n_hits, lag_origin, samples_per_tbin,
                            f_lo_hz, df_hz, n_fbins, n_tbins, map_dev, (unsigned long long *)counters_dev,
                            (cudaStream_t)stream);
@@ -417,7 +478,7 @@ int bfly_butterfly_map(const bfly_bank *bank, const float *rho_max_dev, const in
     if (!std::isfinite(kappa)) { set_error("kappa must be finite"); return BFLY_EINVAL; }
     if (!(df_hz > 0.0) || !std::isfinite(df_hz) || !std::isfinite(f_lo_hz)) { set_error("df must be finite and > 0, f_lo finite"); return BFLY_EINVAL; }
     if (samples_per_tbin <= 0 || n_fbins <= 0 || n_tbins <= 0 || lag_origin < 0) { set_error("bad map geometry"); return BFLY_EINVAL; }
-    BFLY_CUDA(cudaSetDevice(bank->device));
+    BFLY_ENTER(bank);
     return launch_map(bank, rho_max_dev, arg_lag_dev, kappa, lag_origin, samples_per_tbin, f_lo_hz,
                       df_hz, n_fbins, n_tbins, map_dev, (unsigned long long *)counters_dev,
                       (cudaStream_t)stream);
@@ -435,10 +496,12 @@ int bfly_search_host(bfly_bank *b, const float *x_host, int64_t n_samples, int64
     if (chunk_samples <= 0 || chunk_samples > n_samples) chunk_samples = n_samples;
     if (chunk_samples <= b->L && chunk_samples < n_samples) { set_error("chunk_samples must exceed L"); return BFLY_EINVAL; }
     if (chunk_samples >= (1LL << 31)) { set_error("chunk too long"); return BFLY_ERANGE; }
-    BFLY_CUDA(cudaSetDevice(b->device));
+    BFLY_ENTER(b);
+    BFLY_LOCK(b);
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = reserve_for(b, chunk_samples);
+    int rc = ws_begin(b, st);
     if (rc) return rc;
+    if ((rc = reserve_for(b, chunk_samples))) return rc;
     if ((rc = grow(&b->x_stage, &b->x_stage_cap, chunk_samples))) return rc;
     const int64_t cells = (int64_t)n_fbins * n_tbins;
     if ((rc = grow(&b->map_stage, &b->map_stage_cap, cells))) return rc;
@@ -454,11 +517,13 @@ int bfly_search_host(bfly_bank *b, const float *x_host, int64_t n_samples, int64
         const int64_t lag_end = last ? lags_here : (hop < lags_here ? hop : lags_here);
         BFLY_CUDA(cudaMemcpyAsync(b->x_stage, x_host + start, sizeof(float) * (size_t)n,
                                   cudaMemcpyHostToDevice, st));
-        rc = bfly_correlate(b, b->x_stage, n, 0, lag_end, b->rho_stage, b->arg_stage, st);
+        int form = BFLY_FORM_DEFAULT;
+        rc = correlate_check(b, &form, b->x_stage, n, 0, lag_end, b->rho_stage, b->arg_stage);
         if (rc) return rc;
-        rc = bfly_butterfly_map(b, b->rho_stage, b->arg_stage, kappa, start, samples_per_tbin,
-                                f_lo_hz, df_hz, n_fbins, n_tbins, b->map_stage,
-                                (uint64_t *)b->cnt_stage, st);
+        rc = correlate_locked(b, form, b->x_stage, n, 0, lag_end, b->rho_stage, b->arg_stage, st);
+        if (rc) return rc;
+        rc = launch_map(b, b->rho_stage, b->arg_stage, kappa, start, samples_per_tbin, f_lo_hz, df_hz,
+                        n_fbins, n_tbins, b->map_stage, b->cnt_stage, st);
         if (rc) return rc;
         if (last) break;
     }

@@ -388,7 +388,9 @@ int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag
                     float *rho_max, int32_t *arg_lag, cudaStream_t stream)
 {
     static EncodeTiledFn encode = nullptr;
-    static bool attr_set = false;
+    static PerDeviceOnce once;           // function attributes are per device
+    static std::mutex encode_mutex;
+    std::unique_lock<std::mutex> encode_lock(encode_mutex);
     if (!encode) {
         cudaDriverEntryPointQueryResult q;
         void *fn = nullptr;
@@ -396,10 +398,12 @@ int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag
         if (!fn || q != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled is not available"); return BFLY_EUNSUPPORTED; }
         encode = (EncodeTiledFn)fn;
     }
-    if (!attr_set) {
+    encode_lock.unlock();
+    const int rc_attr = once.run(b->device, []() -> int {
         BFLY_CUDA(cudaFuncSetAttribute(dense_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DT_SMEM));
-        attr_set = true;
-    }
+        return BFLY_OK;
+    });
+    if (rc_attr) return rc_attr;
     const int64_t n_lags = lag_end - lag_begin;
     const int64_t n_lag_tiles = (n_lags + DT_N - 1) / DT_N;
     const int64_t n_kb = (b->L + DT_K - 1) / DT_K;

@@ -152,14 +152,15 @@ int64_t fft_blocks_needed(int32_t L, int64_t n_lags)
 int launch_fft(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceOnce once;           // function attributes are per device
+    const int rc_attr = once.run(b->device, []() -> int {
         BFLY_CUDA(cudaFuncSetAttribute(data_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(fft_correlate_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM));
-        attr_set = true;
-    }
+        return BFLY_OK;
+    });
+    if (rc_attr) return rc_attr;
     const int64_t n_lags = lag_end - lag_begin;
     const int32_t V = FFT_B - b->L + 1;
     const int64_t n_blocks = fft_blocks_needed(b->L, n_lags);

@@ -653,20 +653,28 @@ int64_t tc_blocks_needed(int64_t n_lags)
     return nb;
 }
 
-static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
-                            int64_t lag_end, float *rho_max, int32_t *arg_lag, const TailArgs *tails,
-                            cudaStream_t stream)
+// cudaFuncAttributeMaxDynamicSharedMemorySize of every kernel of this file, once per device
+static int tc_attrs(int device)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceOnce once;
+    return once.run(device, []() -> int {
         BFLY_CUDA(cudaFuncSetAttribute(tc_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_wspec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        attr_set = true;
-    }
+        BFLY_CUDA(cudaFuncSetAttribute(tc_debug_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        return BFLY_OK;
+    });
+}
+
+static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                            int64_t lag_end, float *rho_max, int32_t *arg_lag, const TailArgs *tails,
+                            cudaStream_t stream)
+{
+    int rc = tc_attrs(b->device);
+    if (rc) return rc;
     const int64_t n_lags = lag_end - lag_begin;
     if (n_lags >= (1LL << 31) - 2 * TCV) { set_error("too many lags"); return BFLY_ERANGE; }
     int64_t n_blocks; int32_t n_tail;
@@ -723,12 +731,8 @@ int launch_tails_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64
     tc_autocorr_kernel<<<(unsigned)b->L, 256, 0, stream>>>(x, n_samples, b->racf);
     count_launch();
     BFLY_CUDA(cudaGetLastError());
-    // the attribute for tc_wspec_kernel is set in launch_tc_common; make sure it ran once
-    static bool attr_set = false;
-    if (!attr_set) {
-        BFLY_CUDA(cudaFuncSetAttribute(tc_wspec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
-        attr_set = true;
-    }
+    const int rc = tc_attrs(b->device);
+    if (rc) return rc;
     tc_wspec_kernel<<<1, fft32::NT, fft32::FFT_SMEM, stream>>>(b->racf, b->L, b->wspec);
     count_launch();
     BFLY_CUDA(cudaGetLastError());
@@ -747,7 +751,10 @@ int launch_tails_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64
 
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream)
 {
-    BFLY_CUDA(cudaFuncSetAttribute(tc_debug_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+    int dev = 0;
+    BFLY_CUDA(cudaGetDevice(&dev));
+    const int rc = tc_attrs(dev);
+    if (rc) return rc;
     tc_debug_fft_kernel<<<1, NT, TC_SMEM, stream>>>(y, z, full);
     count_launch();
     BFLY_CUDA(cudaGetLastError());

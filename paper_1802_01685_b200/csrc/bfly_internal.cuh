@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
+
 #include "../../include/bfly.h"
 
 struct bfly_bank {
@@ -50,6 +52,14 @@ struct bfly_bank {
     uint32_t *map_stage;
     int64_t map_stage_cap;
     unsigned long long *cnt_stage;  // 2
+    // guards of the mutable workspace: `busy` makes a second host thread entering a
+    // workspace-using call on the same bank fail with BFLY_EINVAL instead of racing; `ws_event`
+    // (recorded at the end of every such call) orders the workspace between streams: a call on
+    // another stream than the previous one first waits for it
+    int busy;
+    cudaEvent_t ws_event;
+    cudaStream_t ws_stream;
+    int ws_valid;
     // measurement aid (bfly_bank_set_timing)
     int timing;
     int timed;                  // a start/stop pair has been recorded
@@ -67,6 +77,52 @@ void count_launch(int n = 1);
         cudaError_t e__ = (call);                                \
         if (e__ != cudaSuccess) return bfly::cuda_fail(e__, #call); \
     } while (0)
+
+// One-time setup that must run once PER DEVICE (cudaFuncSetAttribute applies to the current
+// device's copy of the function only), thread safe.  f() returns a BFLY_* status.
+constexpr int MAX_DEVICES = 64;
+struct PerDeviceOnce {
+    std::mutex m;
+    bool done[MAX_DEVICES] = {};
+    template <class F>
+    int run(int device, F &&f)
+    {
+        if (device < 0 || device >= MAX_DEVICES) { set_error("device %d out of range", device); return BFLY_EINVAL; }
+        std::lock_guard<std::mutex> g(m);
+        if (done[device]) return BFLY_OK;
+        const int rc = f();
+        if (rc == BFLY_OK) done[device] = true;
+        return rc;
+    }
+};
+
+// Every entry point runs on the bank's device and leaves the caller's current device as it was.
+struct DeviceGuard {
+    int prev = -1, dev;
+    cudaError_t err;
+    explicit DeviceGuard(int device) : dev(device)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        err = prev == device ? cudaSuccess : cudaSetDevice(device);
+    }
+    ~DeviceGuard() { if (prev >= 0 && prev != dev) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
+
+// Exclusive use of a bank's workspace for the duration of one call (host side).
+struct BankLock {
+    bfly_bank *b;
+    bool held;
+    explicit BankLock(const bfly_bank *bank) : b(const_cast<bfly_bank *>(bank))
+    {
+        int expected = 0;
+        held = __atomic_compare_exchange_n(&b->busy, &expected, 1, false, __ATOMIC_ACQUIRE, __ATOMIC_RELAXED);
+    }
+    ~BankLock() { if (held) __atomic_store_n(&b->busy, 0, __ATOMIC_RELEASE); }
+    BankLock(const BankLock &) = delete;
+    BankLock &operator=(const BankLock &) = delete;
+};
 
 // bfly_bank_set_timing: events around the correlation-core kernel on the caller's stream
 inline void core_timer_start(const bfly_bank *b, cudaStream_t st)

@@ -109,10 +109,10 @@ def test_lag_subrange_and_empty_range(bfly, form):
 @pytest.mark.parametrize("form", FORMS)
 def test_degenerate_inputs(bfly, form):
     fs, L, N = 1024.0, 512, 3000
-    # (0, 0): the sine template is identically zero and contributes nothing (C4).  (fs/2, 0) is
-    # left out: there the float64 oracle's sin(pi k) is rounding noise, not zero (C4).
-    f0 = np.array([100.0, 0.0, 256.0, 300.0, 511.0])
-    f1 = np.array([50.0, 0.0, 0.0, -700.0, 3.0])
+    # (0, 0) and (fs/2, 0): the sine template is identically zero and contributes nothing (C4);
+    # both sides reduce the phase modulo one turn, so sin(pi k) is exactly 0 on both
+    f0 = np.array([100.0, 0.0, 256.0, 300.0, 511.0, 512.0])
+    f1 = np.array([50.0, 0.0, 0.0, -700.0, 3.0, 0.0])
     # all-zero data: rho = 0 everywhere, argmax = first lag (C6, C8)
     x = np.zeros(N, np.float32)
     _, rho, arg = _run(bfly, form, fs, L, f0, f1, x)

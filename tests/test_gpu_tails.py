@@ -19,8 +19,8 @@ def bfly():
     return b
 
 
-def _tails(bfly, fs, L, f0, f1, x, kappa, capacity, lb=0, le=None):
-    bank = bfly.make_bank(fs, L, f0, f1)
+def _tails(bfly, fs, L, f0, f1, x, kappa, capacity, lb=0, le=None, f2=None):
+    bank = bfly.make_bank(fs, L, f0, f1, f2_hzps2=f2)
     xd = torch.from_numpy(x).cuda()
     sig, hj, hl, hr, n = bfly.tails(bank, xd, kappa, capacity, lb, le)
     torch.cuda.synchronize()
@@ -74,6 +74,47 @@ def test_tails_sub_bank_of_config(bfly, index, n_random, kappa):
     f0, f1 = f0a[idx], f1a[idx]
     bank, sig, hj, hl, hr, total, _ = _tails(bfly, cfg.fs_hz, cfg.L, f0, f1, x, kappa, 1 << 18)
     n_oracle, _ = check_tails(x, cfg.fs_hz, cfg.L, f0, f1, kappa, sig, hj, hl, hr, total)
+    assert n_oracle > 0
+
+
+def test_tails_on_a_cubic_phase_bank(bfly):
+    """bfly_tails on a bfly_make_bank3 bank (tc_correlate_kernel<TAILS, CUBIC>): the kappa-sigma
+    reduction applies to whatever bank is searched.  R5 against oracle.sigma /
+    oracle.rho_series with f2; a curved injection is found at its start by its own template."""
+    rng = np.random.default_rng(27)
+    fs, L, N = 2048.0, 2048, 12000
+    x = rng.standard_normal(N)
+    f0 = np.concatenate([[700.0], rng.uniform(100, 900, 29)])
+    f1 = np.concatenate([[-250.0], rng.uniform(-300, 300, 29)])
+    f2 = np.concatenate([[400.0], rng.uniform(-600, 600, 29)])
+    hc, _ = oracle.template(fs, L, f0[0], f1[0], f2[0])
+    x[5000:5000 + L] += 0.25 * hc
+    x = x.astype(np.float32)
+    kappa = 3.6
+    for lb, le in ((0, None), (1000, 1000 + 2 * 4096 + 3)):
+        _, sig, hj, hl, hr, total, _ = _tails(bfly, fs, L, f0, f1, x, kappa, 1 << 16, lb, le, f2=f2)
+        n_oracle, _ = check_tails(x, fs, L, f0, f1, kappa, sig, hj, hl, hr, total, lb,
+                                  le, f2=f2)
+        assert n_oracle > 30 and 5000 in hl[hj == 0]
+    # f2 = 0 for every template: the cubic bank's tails are those of the linear bank, bit for bit
+    _, sa, ja, la, ra, ta, _ = _tails(bfly, fs, L, f0, f1, x, kappa, 1 << 16)
+    _, sb, jb, lb_, rb, tb, _ = _tails(bfly, fs, L, f0, f1, x, kappa, 1 << 16, f2=np.zeros(30))
+    assert ta == tb and np.array_equal(sa, sb)
+    assert sorted(zip(ja.tolist(), la.tolist(), ra.tolist())) == sorted(zip(jb.tolist(), lb_.tolist(), rb.tolist()))
+
+
+def test_tails_cubic_bank_one_paper_scale_segment(bfly):
+    """One config-4-sized segment (65536 samples, L = 4096, 15 blocks + the 61441st lag) against a
+    cubic-phase sub-bank: R5."""
+    cfg = get_config(4)
+    x = make_data(cfg)
+    rng = np.random.default_rng(28)
+    f0a, f1a = bank_grid(cfg)
+    idx = sub_bank_indices(cfg, 10, max_track=4)
+    f0, f1 = f0a[idx], f1a[idx]
+    f2 = rng.uniform(-400, 400, len(idx))
+    _, sig, hj, hl, hr, total, _ = _tails(bfly, cfg.fs_hz, cfg.L, f0, f1, x, 4.0, 1 << 18, f2=f2)
+    n_oracle, _ = check_tails(x, cfg.fs_hz, cfg.L, f0, f1, 4.0, sig, hj, hl, hr, total, f2=f2)
     assert n_oracle > 0
 
 
