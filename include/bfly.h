@@ -254,6 +254,26 @@ int bfly_bank_core_ms(bfly_bank *bank, float *ms_out);
  * |y| must stay within the fp16 range.  Asynchronous on `stream`. */
 int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream);
 
+/* Measurement aid (bench.py's roofline denominators; "measured by a microbenchmark
+ * on the box"): runs one microbenchmark kernel on every SM of the CURRENT device (two warm-up
+ * launches, the third timed with CUDA events) and returns its rate.  Synchronous.
+ *   BFLY_PEAK_FFMA   value_out[0] = fp32 flop/s of independent FFMA chains (2 flop each)
+ *   BFLY_PEAK_FFMA2  the same with the packed two-lane FFMA2 of sm_100 (4 flop each)
+ *   BFLY_PEAK_LDS    bytes/s of a conflict-free ld.shared.v4 stream
+ *   BFLY_PEAK_HMMA   flop/s of independent mma.sync.m16n8k16 f16 -> f32 (4096 flop each)
+ *   BFLY_PEAK_SHFL   warp shuffles/s
+ *   BFLY_PEAK_L2     bytes/s of ld.global.v4 over a 480 KB set shared by all CTAs (L2-resident)
+ *   BFLY_PEAK_UMMA   value_out must hold 2 doubles: [0] = flop per clock and SM of back-to-back
+ *                    tcgen05.mma kind::f16 M = 128, K = 16 (variant bits 0-1: 1 = A, B from shared
+ *                    memory, 2 = A from tensor memory, 0 = none; bit 2: N = 256 instead of 128),
+ *                    [1] = clocks per iteration of 16 warps streaming beside it (bit 3: 32 KB of
+ *                    st.shared.v4 + 32 KB of ld.shared.v4 per iteration; bit 4: 64 KB of
+ *                    tcgen05.ld per iteration)
+ * `variant` is ignored by the others.  ms_out (optional): the timed launch in milliseconds. */
+enum { BFLY_PEAK_FFMA = 0, BFLY_PEAK_FFMA2 = 1, BFLY_PEAK_LDS = 2, BFLY_PEAK_HMMA = 3,
+       BFLY_PEAK_SHFL = 4, BFLY_PEAK_L2 = 5, BFLY_PEAK_UMMA = 6 };
+int bfly_debug_peak(int which, int variant, int iters, double *value_out, double *ms_out);
+
 /* Number of kernel launches the library has enqueued so far in this process (for bench.py's
  * gpu_launches claim). */
 int64_t bfly_launch_count(void);

@@ -18,9 +18,12 @@ from . import build as _build
 __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
            "butterfly_map", "search_host", "launch_count", "lib_path",
            "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC",
-           "debug_fft_tc", "tails", "hits_map", "time_randomize", "coincidence", "pseudo_spectrum"]
+           "debug_fft_tc", "tails", "hits_map", "time_randomize", "coincidence", "pseudo_spectrum",
+           "debug_peak", "PEAK_FFMA", "PEAK_FFMA2", "PEAK_LDS", "PEAK_HMMA", "PEAK_SHFL", "PEAK_L2",
+           "PEAK_UMMA"]
 
 FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC, FORM_DENSE_TC = 0, 1, 2, 3, 4
+PEAK_FFMA, PEAK_FFMA2, PEAK_LDS, PEAK_HMMA, PEAK_SHFL, PEAK_L2, PEAK_UMMA = range(7)
 
 
 class BflyError(RuntimeError):
@@ -64,13 +67,14 @@ def _load():
     lib.bfly_bank_set_timing.argtypes = [vp, C.c_int]
     lib.bfly_bank_core_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.bfly_debug_fft_tc.argtypes = [vp, vp, C.c_int, vp]
+    lib.bfly_debug_peak.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(f64), C.POINTER(f64)]
     lib.bfly_launch_count.argtypes = []
     lib.bfly_launch_count.restype = i64
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
                  "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
                  "bfly_search_host", "bfly_debug_fft_tc", "bfly_tails", "bfly_hits_map",
                  "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum",
-                 "bfly_make_bank3", "bfly_bank_get_f2"):
+                 "bfly_make_bank3", "bfly_bank_get_f2", "bfly_debug_peak"):
         getattr(lib, name).restype = C.c_int
     return lib, path
 
@@ -357,6 +361,18 @@ def debug_fft_tc(y: torch.Tensor, full: bool = False) -> torch.Tensor:
     _check(_lib.bfly_debug_fft_tc(C.c_void_p(y.data_ptr()), C.c_void_p(z.data_ptr()),
                                   int(bool(full)), _stream(y.device.index)), "bfly_debug_fft_tc")
     return z
+
+
+def debug_peak(which: int, variant: int = 0, iters: int = 2000, device: int = 0):
+    """bfly_debug_peak: one microbenchmark on every SM of `device`.  Returns (value, ms) --
+    value is a float (flop/s, bytes/s or shuffles/s) except for PEAK_UMMA, where it is the pair
+    (MMA flop per clock and SM, clocks per iteration of the streaming warps)."""
+    out = (C.c_double * 2)(0.0, 0.0)
+    ms = C.c_double(0.0)
+    with torch.cuda.device(device):
+        _check(_lib.bfly_debug_peak(int(which), int(variant), int(iters), out, C.byref(ms)),
+               "bfly_debug_peak")
+    return ((out[0], out[1]) if which == PEAK_UMMA else out[0]), ms.value
 
 
 def launch_count() -> int:
