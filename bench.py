@@ -117,11 +117,25 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
+def host_description():
+    """nproc and the CPU model string of the box the CPU baselines ran on."""
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return {"nproc": os.cpu_count(), "cpu_model": model}
+
+
 def time_oracle(cfg, x, f0, f1, seconds):
     """The oracle as it stands on the host cores, on a bounded sample of the workload: as many
     of the given templates (all lags) as fit in about `seconds`.  Returns (corr/s, n, s, cores)."""
     import oracle
-    n0 = min(8, len(f0))
+    n0 = min(64, len(f0))         # several templates per core, so that the first timing is not noise
     t = time.perf_counter()
     oracle.correlate(x, cfg.fs_hz, cfg.L, f0[:n0], f1[:n0])
     dt0 = time.perf_counter() - t
@@ -132,6 +146,22 @@ def time_oracle(cfg, x, f0, f1, seconds):
     return correlations_per_step(cfg, n) / dt, n, dt, oracle.max_threads()
 
 
+def time_oracle_fft(cfg, x, f0, f1, seconds):
+    """The second reported CPU baseline: oracle/fft_variant.py, the float64 numpy
+    FFT restatement of the correlation -- the paper's own algorithm (FFT-based
+    correlation) on the host, as it stands (numpy's pocketfft, one thread)."""
+    from oracle import fft_variant
+    n0 = min(4, len(f0))
+    t = time.perf_counter()
+    fft_variant.correlate_fft(x, cfg.fs_hz, cfg.L, f0[:n0], f1[:n0])
+    dt0 = time.perf_counter() - t
+    n = int(max(n0, min(len(f0), (seconds / max(dt0, 1e-3)) * n0)))
+    t = time.perf_counter()
+    fft_variant.correlate_fft(x, cfg.fs_hz, cfg.L, f0[:n], f1[:n])
+    dt = time.perf_counter() - t
+    return correlations_per_step(cfg, n) / dt, n, dt
+
+
 def run_reference(args, cfg, rank):
     """--impl reference: the float64 oracle on the box's host cores (rank 0 only)."""
     if rank != 0:
@@ -139,13 +169,18 @@ def run_reference(args, cfg, rank):
     import oracle
     x = make_data(cfg)
     f0a, f1a = bank_grid(cfg)
-    idx = sub_bank_indices(cfg, 4096, seed=7, halfwidth=0, max_track=0)
+    idx = sub_bank_indices(cfg, 1 << 16, seed=7, halfwidth=0, max_track=0)
     f0, f1 = f0a[idx], f1a[idx]
-    # size one step at about 8 s of CPU work
+    # one step = a bounded sample: about 150 s of CPU work for the whole run, at most 8 s per step,
+    # in whole multiples of the thread count (the oracle hands out templates one by one)
+    cores = oracle.max_threads()
+    n0 = 4 * cores
     t = time.perf_counter()
-    oracle.correlate(x, cfg.fs_hz, cfg.L, f0[:8], f1[:8])
-    per8 = time.perf_counter() - t
-    n = int(max(8, min(len(f0) // max(args.steps + args.warmup, 1), 8.0 / max(per8, 1e-3) * 8)))
+    oracle.correlate(x, cfg.fs_hz, cfg.L, f0[:n0], f1[:n0])
+    per_template = (time.perf_counter() - t) / n0
+    step_s = min(8.0, 150.0 / max(args.steps + args.warmup, 1))
+    n = int(step_s / max(per_template, 1e-6)) // cores * cores
+    n = max(cores, min(len(f0) // max(args.steps + args.warmup, 1), n))
     pos = 0
     for _ in range(args.warmup):
         oracle.correlate(x, cfg.fs_hz, cfg.L, f0[pos:pos + n], f1[pos:pos + n]); pos += n
@@ -163,9 +198,27 @@ def run_reference(args, cfg, rank):
         "config": {"workload": f"config {cfg.index} ({cfg.name})", "templates_per_step": n,
                    "n_samples": cfg.n_samples, "L": cfg.L, "lags": cfg.n_lags},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(),
-                         "kind": "oracle", "sample": sample},
+                         "kind": "oracle", "sample": sample, **host_description()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
+
+
+def measure_peaks(bfly, device):
+    """The unit rates the correlation kernels are bound by, measured on this box in this run
+    (bfly_debug_peak; "measured by a microbenchmark on the box")."""
+    ffma, _ = bfly.debug_peak(bfly.PEAK_FFMA, 0, 4000, device)
+    ffma2, _ = bfly.debug_peak(bfly.PEAK_FFMA2, 0, 4000, device)
+    lds, _ = bfly.debug_peak(bfly.PEAK_LDS, 0, 4000, device)
+    hmma, _ = bfly.debug_peak(bfly.PEAK_HMMA, 0, 4000, device)
+    l2, _ = bfly.debug_peak(bfly.PEAK_L2, 0, 2000, device)
+    (umma_ss, _), _ = bfly.debug_peak(bfly.PEAK_UMMA, 1 | 4, 3000, device)
+    (umma_ts, _), _ = bfly.debug_peak(bfly.PEAK_UMMA, 2 | 4, 3000, device)
+    return {"ffma_tflops": ffma / 1e12, "ffma2_tflops": ffma2 / 1e12, "lds_tbs": lds / 1e12,
+            "hmma_tflops": hmma / 1e12, "l2_hot_tbs": l2 / 1e12,
+            "tcgen05_f16_m128n256_smem_a_flop_per_clk_sm": umma_ss,
+            "tcgen05_f16_m128n256_tmem_a_flop_per_clk_sm": umma_ts,
+            "how": "bfly_debug_peak (csrc/bfly_peaks.cu): one kernel per unit on every SM, CUDA events, "
+                   "third of three launches"}
 
 
 def main():
@@ -274,48 +327,82 @@ def main():
                "d2h_bytes_per_step": int(T * 8 + m.numel() * 4 + 16)}
 
     if rank == 0:
-        # ---- roofline of the dominant kernel (the correlation core), timed live above
-        core_s = float(np.mean(core_ms)) * 1e-3
+        # ---- roofline of the dominant kernel (the correlation core), timed live above; every
+        #      denominator is measured in this run by bfly_debug_peak
+        core_s = float(np.median(core_ms)) * 1e-3
         is_fft = form in (0, 1, 3)
         is_tc = form in (0, 3) and cfg.L >= 256           # BFLY_TC_MIN_L (include/bfly.h)
         is_dense = form == 4
-        flops = fft_form_flops(cfg, T) if is_fft else direct_form_flops(cfg, T)
-        peak_tflops = SM_COUNT * FP32_LANES * 2 * 1.965e9 / 1e12
-        achieved = flops / core_s / 1e12
         kernel = (("tc_correlate_kernel" if is_tc else "fft_correlate_kernel") if is_fft
                   else "dense_tc_kernel" if is_dense else "direct_kernel")
-        peaks = {}
-        ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
-        if os.path.exists(ppath):
-            peaks = json.load(open(ppath))
-        bf16 = peaks.get("bf16_tflops_sustained", 1400.0)
+        peaks = measure_peaks(bfly, local)
+        mpath = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        driver_peaks = json.load(open(mpath)) if os.path.exists(mpath) else {}
+        bf16 = driver_peaks.get("bf16_tflops_sustained", 1400.0)
         bf16_basis = ("measured sustained cuBLAS bf16 (MEASURED_PEAKS.json); fp16 operands run at the same rate"
-                      if peaks else "fallback 1.4 PFLOP/s sustained")
-        traffic = None
+                      if driver_peaks else "fallback 1.4 PFLOP/s sustained (B200_PROFILING.md)")
+        alg_flops = fft_form_flops(cfg, T) if is_fft else direct_form_flops(cfg, T)
+        fp32_peak = peaks["ffma_tflops"]
+        algorithmic = {"flops_per_launch": alg_flops, "tflops": alg_flops / core_s / 1e12,
+                       "fp32_fma_peak_tflops_measured": fp32_peak,
+                       "ratio_to_fp32_peak": alg_flops / core_s / 1e12 / fp32_peak,
+                       "basis": ("(n_blocks + 1) x 5 B log2 B + n_blocks x 6 B per template, B = 8192 "
+                                 "(SURVEY 8(d)); the rate a CUDA-core FFT would need -- a yardstick, "
+                                 "not the pipe this kernel runs on") if is_fft
+                                else "2 quadratures x 2 L n_lags flop per template (SURVEY 8(d))"}
+        traffic, traffic_src = None, None
         tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
         if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get(kernel + "_bytes_per_launch")
-        roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                    "frac": achieved / peak_tflops, "traffic": traffic,
-                    "kernel": kernel,
-                    "kernel_ms": core_s * 1e3, "kernel_share_of_step": core_s * 1e3 * args.steps / ms,
-                    "flops_per_launch": flops,
-                    "flops_basis": "algorithmic FFT-form flops: (n_blocks + 1) x 5 B log2 B + n_blocks x 6 B "
-                                   "per template, B = 8192" if is_fft else "2 x 2 L n_lags per template",
-                    "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz"}
-        if is_dense:
-            roofline.update({"bound": "tensor", "peak": bf16, "frac": achieved / bf16, "peak_basis": bf16_basis,
-                             "flops_basis": "2 quadratures x 2 L n_lags flop per template (one pass, fp16 operands)"})
+            tj = json.load(open(tpath))
+            per_template = tj.get(kernel + "_bytes_per_template")
+            if per_template is not None:
+                traffic = per_template * T
+                traffic_src = tj.get(kernel + "_source")
         if is_tc:
-            # what the tensor pipe actually executes: 512 (+256 for G's upper rows) m16n8k16 MMAs
-            # of 4096 flop per length-8192 transform
-            n_blocks = -(-(cfg.n_lags - 4) // 4096)
+            # what the kernel executes on its binding units: mma.sync m16n8k16 MMAs
+            # (4096 flop each): 512 per block transform, 768 for G; shared-memory bytes: per block
+            # X_b staged and read, G read, one exchange written and read (5 x 32 KB), per template
+            # g's exchange, G written (3 x 32 KB) and the tail window
+            n_blocks, n_tail = divmod(cfg.n_lags, 4096)      # tc_plan (csrc/bfly_fft_tc.cu)
+            if n_tail > 4:
+                n_blocks, n_tail = n_blocks + 1, 0
             mma_flops = T * (n_blocks * 512 + 768) * 4096
-            roofline["tensor"] = {"executed_tflops": mma_flops / core_s / 1e12,
-                                  "peak": bf16, "frac": mma_flops / core_s / 1e12 / bf16,
-                                  "peak_basis": bf16_basis,
-                                  "note": "dense flops of the real-embedded DFT matrices on mma.sync "
-                                          "fp16; not algorithmic work"}
+            smem_bytes = T * (n_blocks * 5 * 32768 + 3 * 32768 + (cfg.L * 4 * n_tail))
+            t_hmma = mma_flops / (peaks["hmma_tflops"] * 1e12)
+            t_smem = smem_bytes / (peaks["lds_tbs"] * 1e12)
+            tight = max(t_hmma, t_smem)
+            roofline = {"bound": "tensor", "kernel": kernel,
+                        "achieved": mma_flops / core_s / 1e12, "peak": peaks["hmma_tflops"],
+                        "unit": "TFLOP/s", "frac": mma_flops / core_s / 1e12 / peaks["hmma_tflops"],
+                        "flops_per_launch": mma_flops,
+                        "flops_basis": "executed: (512 n_blocks + 768) mma.sync.m16n8k16 x 4096 flop per template "
+                                       "(the real-embedded radix-8/16 DFT matrices of the FFT; DESIGN.md 6.1)",
+                        "peak_basis": "measured in this run (bfly_debug_peak): independent mma.sync.m16n8k16 "
+                                      "f16->f32 on every SM, the pipe this kernel's MMAs run on",
+                        "bounds_s": {"mma_sync": t_hmma, "shared_memory": t_smem},
+                        "smem_bytes_per_launch": smem_bytes,
+                        "frac_of_tightest_bound": tight / core_s,
+                        "tightest_bound": "shared_memory" if t_smem >= t_hmma else "mma_sync",
+                        "vs_tcgen05_rate": {"frac": mma_flops / core_s / 1e12 / bf16, "peak": bf16,
+                                            "peak_basis": bf16_basis}}
+        elif is_dense:
+            roofline = {"bound": "tensor", "kernel": kernel, "achieved": alg_flops / core_s / 1e12,
+                        "peak": bf16, "unit": "TFLOP/s", "frac": alg_flops / core_s / 1e12 / bf16,
+                        "flops_per_launch": alg_flops, "flops_basis": algorithmic["basis"],
+                        "peak_basis": bf16_basis}
+        else:
+            roofline = {"bound": "alu", "kernel": kernel, "achieved": alg_flops / core_s / 1e12,
+                        "peak": fp32_peak, "unit": "TFLOP/s", "frac": alg_flops / core_s / 1e12 / fp32_peak,
+                        "flops_per_launch": alg_flops, "flops_basis": algorithmic["basis"],
+                        "peak_basis": "measured in this run (bfly_debug_peak): independent FFMA chains on every SM"}
+        roofline.update({"traffic": traffic, "traffic_source": traffic_src,
+                         "algorithmic_bytes_per_launch": T * 32,
+                         "kernel_ms": core_s * 1e3, "kernel_ms_all": [float(v) for v in core_ms],
+                         "kernel_share_of_step": core_s * 1e3 * args.steps / ms,
+                         "algorithmic": algorithmic, "peaks_measured": peaks})
+        npath = os.path.join(ROOT, "profiles", "ncu_utilisation.json")
+        if os.path.exists(npath):
+            roofline["ncu"] = json.load(open(npath)).get(kernel)
         f0a, f1a = bank_grid(cfg)
         # ---- the other tensor-core form beside the chosen one ("chosen by measurement"): the dense
         #      tcgen05 contraction on the first 4 waves of template tiles (cost is linear in T)
@@ -357,6 +444,7 @@ def main():
         # ---- the oracle beside it, on this box's host cores, on a bounded sample
         idx = sub_bank_indices(cfg, 8192, seed=7, halfwidth=0, max_track=0)
         cv, cn, cs, cores = time_oracle(cfg, x, f0a[idx], f1a[idx], args.cpu_seconds)
+        fv, fn, fs_ = time_oracle_fft(cfg, x, f0a[idx], f1a[idx], min(args.cpu_seconds, 15.0))
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -376,7 +464,12 @@ def main():
             "direct_equiv_mac_per_s": world * T * cfg.n_lags * 2 * cfg.L * args.steps / (ms * 1e-3),
             "cpu_baseline": {"value": cv, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": f"{cn} templates x all {cfg.n_lags} lags of config "
-                                       f"{cfg.index} in {cs:.1f} s (float64 direct)"},
+                                       f"{cfg.index} in {cs:.1f} s (float64 direct, OpenMP)",
+                             **host_description()},
+            "cpu_baseline_fft": {"value": fv, "unit": UNIT, "cores": 1, "kind": "oracle (float64 FFT variant)",
+                                 "sample": f"{fn} templates x all {cfg.n_lags} lags in {fs_:.1f} s "
+                                           "(oracle/fft_variant.py: numpy FFT correlation, the paper's "
+                                           "algorithm, PAPER.md:70, one thread)"},
         }
         print(json.dumps(out))
     if world > 1:

@@ -117,6 +117,33 @@ int bfly_make_bank_grid(double fs_hz, int32_t L,
 void bfly_free_bank(bfly_bank *bank);            /* NULL is allowed */
 int64_t bfly_bank_size(const bfly_bank *bank);   /* number of templates; -1 if bank is NULL */
 
+/* Template families.  BFLY_FAMILY_POLY: polynomial phase (f0, f1 [, f2]) -- bfly_make_bank,
+ * bfly_make_bank3, bfly_make_bank_grid.  BFLY_FAMILY_SETTLE: exponentially settling chirps,
+ * bfly_make_bank_settle below. */
+enum { BFLY_FAMILY_POLY = 0, BFLY_FAMILY_SETTLE = 1 };
+
+/* ---- A1 for the settling family (reading N2 of DESIGN.md) ---------------
+ * PAPER.md:21-26 (sec. 1, Eq. 1: descending chirps of a spinning-down black hole-disk system that
+ * "reach a late time plateau" f_GW = 600-700 Hz (M/10 Msun)^-1), PAPER.md:60 (Fig. 2, right) and
+ * PAPER.md:54 ("trajectories of frequency f(t)"); the paper prints no waveform, the reading is
+ *     f(t) = f_inf + D exp(-t / tc),   phi_k = 2 pi ( f_inf t_k + D tc (1 - exp(-t_k / tc)) ),
+ * t_k = k/fs, k = 0 .. L-1: D = f(0) - f_inf [Hz] (D > 0 descends towards the plateau f_inf), tc > 0
+ * the settling time [s].  f_inf_hz, delta_hz, tau_c_s: HOST, n_templates float64 each.  The rest of
+ * the path is unchanged: every correlation form, bfly_tails, the maps.  The butterfly map bins a
+ * template by its START frequency f_inf + D (reading C10: the frequency the signal has at the
+ * start of the matched window); bfly_bank_get returns that as f0, with f1 = -D/tc and
+ * bfly_bank_get_f2 = D/tc^2 (slope and curvature at the first sample).  Errors as bfly_make_bank;
+ * BFLY_EINVAL also for tc <= 0 or a non-finite parameter. */
+int bfly_make_bank_settle(double fs_hz, int32_t L, int64_t n_templates, const double *f_inf_hz,
+                          const double *delta_hz, const double *tau_c_s, int device,
+                          bfly_bank **out_bank);
+/* The family of a bank (BFLY_FAMILY_*; -1 for a null bank), and the parameters of templates
+ * [first, first + count) of a settling bank (HOST outputs, any may be NULL; BFLY_EINVAL for a
+ * bank of the other family). */
+int bfly_bank_family(const bfly_bank *bank);
+int bfly_bank_get_settle(const bfly_bank *bank, int64_t first, int64_t count, double *f_inf_hz,
+                         double *delta_hz, double *tau_c_s);
+
 /* Copy bank parameters of templates [first, first + count) to HOST arrays (any may be NULL):
  * f0, f1 (float64) and the stored 1/||cos phi||^2, 1/||sin phi||^2 (float32).  Synchronous. */
 int bfly_bank_get(const bfly_bank *bank, int64_t first, int64_t count,

@@ -19,10 +19,11 @@ __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "cor
            "butterfly_map", "search_host", "launch_count", "lib_path",
            "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC",
            "debug_fft_tc", "tails", "hits_map", "time_randomize", "coincidence", "pseudo_spectrum",
-           "debug_peak", "PEAK_FFMA", "PEAK_FFMA2", "PEAK_LDS", "PEAK_HMMA", "PEAK_SHFL", "PEAK_L2",
+           "make_bank_settle", "FAMILY_POLY", "FAMILY_SETTLE", "debug_peak", "PEAK_FFMA", "PEAK_FFMA2", "PEAK_LDS", "PEAK_HMMA", "PEAK_SHFL", "PEAK_L2",
            "PEAK_UMMA"]
 
 FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC, FORM_DENSE_TC = 0, 1, 2, 3, 4
+FAMILY_POLY, FAMILY_SETTLE = 0, 1
 PEAK_FFMA, PEAK_FFMA2, PEAK_LDS, PEAK_HMMA, PEAK_SHFL, PEAK_L2, PEAK_UMMA = range(7)
 
 
@@ -46,6 +47,9 @@ def _load():
     lib.bfly_make_bank.argtypes = [f64, i32, i64, vp, vp, C.c_int, C.POINTER(vp)]
     lib.bfly_make_bank3.argtypes = [f64, i32, i64, vp, vp, vp, C.c_int, C.POINTER(vp)]
     lib.bfly_bank_get_f2.argtypes = [vp, i64, i64, vp]
+    lib.bfly_make_bank_settle.argtypes = [f64, i32, i64, vp, vp, vp, C.c_int, C.POINTER(vp)]
+    lib.bfly_bank_get_settle.argtypes = [vp, i64, i64, vp, vp, vp]
+    lib.bfly_bank_family.argtypes = [vp]
     lib.bfly_make_bank_grid.argtypes = [f64, i32, f64, f64, i32, f64, f64, i32, C.c_int,
                                         C.POINTER(vp)]
     lib.bfly_free_bank.argtypes = [vp]
@@ -74,7 +78,8 @@ def _load():
                  "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
                  "bfly_search_host", "bfly_debug_fft_tc", "bfly_tails", "bfly_hits_map",
                  "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum",
-                 "bfly_make_bank3", "bfly_bank_get_f2", "bfly_debug_peak"):
+                 "bfly_make_bank3", "bfly_bank_get_f2", "bfly_debug_peak", "bfly_make_bank_settle",
+                 "bfly_bank_get_settle", "bfly_bank_family"):
         getattr(lib, name).restype = C.c_int
     return lib, path
 
@@ -148,6 +153,18 @@ class Bank:
         _check(_lib.bfly_bank_get_f2(self._h, first, count, f2.ctypes.data), "bfly_bank_get_f2")
         return f2
 
+    @property
+    def family(self) -> int:
+        return int(_lib.bfly_bank_family(self._h))
+
+    def get_settle(self, first: int = 0, count: int | None = None):
+        """(f_inf, D, tc) of templates [first, first+count) of a settling-family bank."""
+        count = len(self) - first if count is None else count
+        a, b, c = (np.empty(count, np.float64) for _ in range(3))
+        _check(_lib.bfly_bank_get_settle(self._h, first, count, a.ctypes.data, b.ctypes.data,
+                                         c.ctypes.data), "bfly_bank_get_settle")
+        return a, b, c
+
     def set_timing(self, enable: bool):
         _check(_lib.bfly_bank_set_timing(self._h, int(bool(enable))), "bfly_bank_set_timing")
 
@@ -178,6 +195,19 @@ def make_bank(fs_hz: float, L: int, f0_hz, f1_hzps, device: int = 0, f2_hzps2=No
             raise ValueError("f2 must have the shape of f0")
         _check(_lib.bfly_make_bank3(float(fs_hz), int(L), f0.size, f0.ctypes.data, f1.ctypes.data,
                                     f2.ctypes.data, int(device), C.byref(h)), "bfly_make_bank3")
+    return Bank(h, int(device), fs_hz, L)
+
+
+def make_bank_settle(fs_hz: float, L: int, f_inf_hz, delta_hz, tau_c_s, device: int = 0) -> Bank:
+    """bfly_make_bank_settle: exponentially settling chirps f(t) = f_inf + D exp(-t/tc)."""
+    a = np.ascontiguousarray(f_inf_hz, dtype=np.float64)
+    b = np.ascontiguousarray(delta_hz, dtype=np.float64)
+    c = np.ascontiguousarray(tau_c_s, dtype=np.float64)
+    if a.ndim != 1 or a.shape != b.shape or a.shape != c.shape:
+        raise ValueError("f_inf, D and tc must be 1-D and of equal length")
+    h = C.c_void_p()
+    _check(_lib.bfly_make_bank_settle(float(fs_hz), int(L), a.size, a.ctypes.data, b.ctypes.data,
+                                      c.ctypes.data, int(device), C.byref(h)), "bfly_make_bank_settle")
     return Bank(h, int(device), fs_hz, L)
 
 

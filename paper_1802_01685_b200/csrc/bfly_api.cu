@@ -137,6 +137,7 @@ void bfly_free_bank(bfly_bank *b)
     cudaFree(b->inc2); cudaFree(b->ins2); cudaFree(b->rn2); cudaFree(b->xspec);
     cudaFree(b->xh); cudaFree(b->rn2p); cudaFree(b->qs);
     cudaFree(b->ys); cudaFree(b->rn2s); cudaFree(b->maxbits); cudaFree(b->racf); cudaFree(b->wspec);
+    cudaFree(b->s_finf); cudaFree(b->s_delta); cudaFree(b->s_tc);
     cudaFree(b->packed); cudaFree(b->x_stage); cudaFree(b->rho_stage); cudaFree(b->arg_stage);
     cudaFree(b->map_stage); cudaFree(b->cnt_stage);
     if (b->ws_event) cudaEventDestroy(b->ws_event);
@@ -206,6 +207,72 @@ int bfly_make_bank3(double fs_hz, int32_t L, int64_t n_templates, const double *
     }
     if (rc) { bfly_free_bank(b); return rc; }
     *out_bank = b;
+    return BFLY_OK;
+}
+
+int bfly_bank_family(const bfly_bank *b) { return b ? b->family : -1; }
+
+int bfly_make_bank_settle(double fs_hz, int32_t L, int64_t n_templates, const double *f_inf_hz,
+                          const double *delta_hz, const double *tau_c_s, int device, bfly_bank **out_bank)
+{
+    if (!out_bank || !f_inf_hz || !delta_hz || !tau_c_s) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (!(fs_hz > 0.0) || !std::isfinite(fs_hz)) { set_error("fs must be finite and > 0"); return BFLY_EINVAL; }
+    if (L < 2) { set_error("L must be >= 2"); return BFLY_EINVAL; }
+    if (L > FFT_MAX_L) { set_error("L = %d exceeds the supported maximum %d", L, FFT_MAX_L); return BFLY_ERANGE; }
+    if (n_templates < 1) { set_error("n_templates must be >= 1"); return BFLY_EINVAL; }
+    std::vector<double> f0, f1, f2;
+    try { f0.resize((size_t)n_templates); f1.resize((size_t)n_templates); f2.resize((size_t)n_templates); }
+    catch (...) { set_error("host allocation failed"); return BFLY_ENOMEM; }
+    for (int64_t j = 0; j < n_templates; ++j) {
+        const double fi = f_inf_hz[j], d = delta_hz[j], tc = tau_c_s[j];
+        if (!std::isfinite(fi) || !std::isfinite(d) || !std::isfinite(tc) || !(tc > 0.0) ||
+            !std::isfinite(d * tc) || !std::isfinite(1.0 / (fs_hz * tc))) {
+            set_error("template %lld: f_inf, D must be finite and tc finite and > 0", (long long)j);
+            return BFLY_EINVAL;
+        }
+        f0[(size_t)j] = fi + d;              // frequency, slope and curvature at the first sample
+        f1[(size_t)j] = -d / tc;
+        f2[(size_t)j] = d / (tc * tc);
+    }
+    // the polynomial bank of the first-sample Taylor coefficients carries f0/f1/f2 (map frequency,
+    // bfly_bank_get); its phase constants and norms are then replaced by the settling family's
+    bfly_bank *b = nullptr;
+    int rc = bfly_make_bank3(fs_hz, L, n_templates, f0.data(), f1.data(), f2.data(), device, &b);
+    if (rc) return rc;
+    DeviceGuard guard(device);
+    const size_t bytes = (size_t)n_templates * sizeof(double);
+    cudaError_t e;
+#define SETTLE_TRY(call) if ((e = (call)) != cudaSuccess) { rc = cuda_fail(e, #call); bfly_free_bank(b); return rc; }
+    SETTLE_TRY(cudaMalloc((void **)&b->s_finf, bytes));
+    SETTLE_TRY(cudaMalloc((void **)&b->s_delta, bytes));
+    SETTLE_TRY(cudaMalloc((void **)&b->s_tc, bytes));
+    SETTLE_TRY(cudaMemcpy(b->s_finf, f_inf_hz, bytes, cudaMemcpyHostToDevice));
+    SETTLE_TRY(cudaMemcpy(b->s_delta, delta_hz, bytes, cudaMemcpyHostToDevice));
+    SETTLE_TRY(cudaMemcpy(b->s_tc, tau_c_s, bytes, cudaMemcpyHostToDevice));
+#undef SETTLE_TRY
+    b->family = BFLY_FAMILY_SETTLE;
+    b->has_f2 = 0;
+    rc = launch_bank_params_settle(b, 0);
+    if (rc == BFLY_OK) {
+        e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) rc = cuda_fail(e, "settle bank parameter kernel");
+    }
+    if (rc) { bfly_free_bank(b); return rc; }
+    *out_bank = b;
+    return BFLY_OK;
+}
+
+int bfly_bank_get_settle(const bfly_bank *b, int64_t first, int64_t count, double *f_inf_hz,
+                         double *delta_hz, double *tau_c_s)
+{
+    if (!b) { set_error("null bank"); return BFLY_EINVAL; }
+    if (b->family != BFLY_FAMILY_SETTLE) { set_error("not a settling-family bank"); return BFLY_EINVAL; }
+    if (first < 0 || count < 0 || first + count > b->T) { set_error("template range outside the bank"); return BFLY_EINVAL; }
+    BFLY_ENTER(b);
+    const size_t n = (size_t)count * sizeof(double);
+    if (f_inf_hz) BFLY_CUDA(cudaMemcpy(f_inf_hz, b->s_finf + first, n, cudaMemcpyDeviceToHost));
+    if (delta_hz) BFLY_CUDA(cudaMemcpy(delta_hz, b->s_delta + first, n, cudaMemcpyDeviceToHost));
+    if (tau_c_s) BFLY_CUDA(cudaMemcpy(tau_c_s, b->s_tc + first, n, cudaMemcpyDeviceToHost));
     return BFLY_OK;
 }
 

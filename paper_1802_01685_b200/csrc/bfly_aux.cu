@@ -57,6 +57,60 @@ __global__ void __launch_bounds__(256) bank_params_kernel(int64_t T, int32_t L, 
     }
 }
 
+// The same for the settling family (reading N2): phA = f_inf/fs as 2^-64 fixed point, phB / phC =
+// the bits of the doubles D tc and 1/(fs tc); norms from the same phase function the kernels use.
+__global__ void __launch_bounds__(256) bank_params_settle_kernel(int64_t T, int32_t L, double fs,
+                                                                 const double *__restrict__ f_inf,
+                                                                 const double *__restrict__ delta,
+                                                                 const double *__restrict__ tc,
+                                                                 uint64_t *__restrict__ phA,
+                                                                 uint64_t *__restrict__ phB,
+                                                                 uint64_t *__restrict__ phC,
+                                                                 float *__restrict__ inc2,
+                                                                 float *__restrict__ ins2)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t j = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (j >= T) return;
+    double a = f_inf[j] / fs;
+    a -= floor(a);
+    if (a >= 1.0) a = 0.0;
+    const uint64_t A = __double2ull_rn(a * 18446744073709551616.0);
+    const double Dtc = delta[j] * tc[j], inv = 1.0 / (fs * tc[j]);
+    double sc = 0.0, ss = 0.0;
+    for (int32_t k = lane; k < L; k += 32) {
+        const uint64_t ph = settle_phase(A, Dtc, inv, (uint64_t)k);
+        const double fr = (double)(int64_t)ph * 5.421010862427522e-20;   // 2^-64
+        double s, c;
+        sincospi(2.0 * fr, &s, &c);
+        sc += c * c;
+        ss += s * s;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        sc += __shfl_xor_sync(0xffffffffu, sc, o);
+        ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    }
+    if (lane == 0) {
+        phA[j] = A;
+        phB[j] = (uint64_t)__double_as_longlong(Dtc);
+        phC[j] = (uint64_t)__double_as_longlong(inv);
+        inc2[j] = sc > 0.0 ? (float)(1.0 / sc) : 0.0f;
+        ins2[j] = ss > 0.0 ? (float)(1.0 / ss) : 0.0f;
+    }
+}
+
+int launch_bank_params_settle(bfly_bank *b, cudaStream_t stream)
+{
+    const int warps = 8;
+    const int64_t blocks = (b->T + warps - 1) / warps;
+    if (blocks >= (1LL << 31)) { set_error("bank too large"); return BFLY_ERANGE; }
+    bank_params_settle_kernel<<<(unsigned)blocks, warps * 32, 0, stream>>>(
+        b->T, b->L, b->fs, b->s_finf, b->s_delta, b->s_tc, b->phA, b->phB, b->phC, b->inc2, b->ins2);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    return BFLY_OK;
+}
+
 int launch_bank_params(bfly_bank *b, cudaStream_t stream)
 {
     const int warps = 8;

@@ -174,7 +174,7 @@ __global__ void dense_prep_kernel(const float *__restrict__ x, int64_t n_samples
 // ------------------------------------------------------------------------------------------
 // The contraction.  Grid: persistent, one CTA per SM, strided over tiles of 128 templates.
 __global__ void __launch_bounds__(DT_THREADS, 1)
-dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
+dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, int family,
                 const uint64_t *__restrict__ phA, const uint64_t *__restrict__ phB,
                 const uint64_t *__restrict__ phC, const float *__restrict__ inc2, const float *__restrict__ ins2,
                 const float *__restrict__ rn2s, int64_t n_lags, int32_t n_lag_tiles,
@@ -227,7 +227,6 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
             const bool valid = j < T;
             const uint64_t A = valid ? phA[j] : 0ull, Bq = valid ? phB[j] : 0ull, Cq = valid ? phC[j] : 0ull;
             const float ic = valid ? inc2[j] : 0.0f, is = valid ? ins2[j] : 0.0f;
-            const uint32_t d3 = (uint32_t)((6ull * Cq) >> 32);     // third difference of the phase (reading N1)
             unsigned long long best = 0ull;
             for (int32_t lt = 0; lt < n_lag_tiles; ++lt) {
                 for (int32_t kb = 0; kb < n_kb; ++kb) {
@@ -237,14 +236,19 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L,
                         bar_expect_tx(full(stage), DT_B_BYTES);
                         tma_load_3d(st + 2 * DT_A_BYTES, &xmap, 0, (lt * DT_N + kb * DT_K) / 8, 0, full(stage));
                     }
-                    // phase of this thread's first sample and its first two differences, exact to
+                    // phase of this thread's first sample and its first three differences, exact to
                     // 2^-32 cycle, then a third-order recurrence in 32-bit fixed point (wrap = mod 1
-                    // cycle; the third difference 6 C is constant, 0 for a linear chirp).  Half a cycle is added so that the bit pattern 0x3F800000 | (ph >> 9),
+                    // cycle; the third difference is the constant 6 C of a cubic phase, 0 for a
+                    // linear chirp; for the settling family (reading N2) it is taken from four exact
+                    // phases and held over the 32 samples: fourth-difference error < 1e-8 cycle).  Half a cycle is added so that the bit pattern 0x3F800000 | (ph >> 9),
                     // a float in [1, 2), minus 1.5 is the phase in [-1/2, 1/2) cycles: no
                     // int-to-float conversion (those share the XU pipe with sin / cos).
                     const uint64_t k0 = (uint64_t)kb * DT_K + 32u * (uint32_t)half;
-                    const uint64_t p0 = template_phase(A, Bq, Cq, k0), p1 = template_phase(A, Bq, Cq, k0 + 1),
-                                   p2 = template_phase(A, Bq, Cq, k0 + 2);
+                    const uint64_t p0 = family_phase(family, A, Bq, Cq, k0), p1 = family_phase(family, A, Bq, Cq, k0 + 1),
+                                   p2 = family_phase(family, A, Bq, Cq, k0 + 2);
+                    const uint32_t d3 = family == BFLY_FAMILY_SETTLE
+                        ? (uint32_t)((family_phase(family, A, Bq, Cq, k0 + 3) - 3ull * p2 + 3ull * p1 - p0) >> 32)
+                        : (uint32_t)((6ull * Cq) >> 32);
                     uint32_t ph = (uint32_t)(p0 >> 32) ^ 0x80000000u;
                     uint32_t d = (uint32_t)((p1 - p0) >> 32);
                     uint32_t dd = (uint32_t)((p2 - 2ull * p1 + p0) >> 32);
@@ -440,7 +444,7 @@ int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag
     const int64_t ctas = std::min<int64_t>(n_ttiles, b->sm_count);
     core_timer_start(b, stream);
     dense_tc_kernel<<<(unsigned)ctas, DT_THREADS, DT_SMEM, stream>>>(
-        map, b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->rn2s, n_lags, (int32_t)n_lag_tiles, lag_begin,
+        map, b->T, b->L, b->family, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->rn2s, n_lags, (int32_t)n_lag_tiles, lag_begin,
         rho_max, arg_lag);
     core_timer_stop(b, stream);
     count_launch();

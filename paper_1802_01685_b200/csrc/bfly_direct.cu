@@ -17,7 +17,7 @@ constexpr int DT_K = 64;     // template samples per chunk
 constexpr int DT_THREADS = 256;
 
 __global__ void __launch_bounds__(DT_THREADS)
-direct_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
+direct_kernel(int64_t T, int32_t L, int family, const uint64_t *__restrict__ phA,
               const uint64_t *__restrict__ phB, const uint64_t *__restrict__ phC,
               const float *__restrict__ inc2,
               const float *__restrict__ ins2, const float *__restrict__ x, int64_t n_samples,
@@ -53,7 +53,7 @@ direct_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             const int j = e / DT_K, kk = e - j * DT_K;
             const int k = k0 + kk;
             float s = 0.0f, c = 0.0f;
-            if (k < L && j0 + j < T) template_sincos(phA[j0 + j], phB[j0 + j], phC[j0 + j], (uint32_t)k, &s, &c);
+            if (k < L && j0 + j < T) template_sincos(family, phA[j0 + j], phB[j0 + j], phC[j0 + j], (uint32_t)k, &s, &c);
             hc[e] = c;
             hs[e] = s;
         }
@@ -137,7 +137,7 @@ int launch_direct(const bfly_bank *b, const float *x, int64_t n_samples, int64_t
         const size_t smem = sizeof(float) * (size_t)(((DT_LAGS + b->L + 3) & ~3) + 2 * DT_J * DT_K);
         core_timer_start(b, stream);
         direct_kernel<<<(unsigned)tiles, DT_THREADS, smem, stream>>>(
-            b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, x, n_samples, lag_begin, n_lags, b->rn2,
+            b->T, b->L, b->family, b->phA, b->phB, b->phC, b->inc2, b->ins2, x, n_samples, lag_begin, n_lags, b->rn2,
             n_lag_tiles, b->packed);
         core_timer_stop(b, stream);
         count_launch();

@@ -60,7 +60,7 @@ data_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_
 // butterflies in the last pass and their epilogue are dead code (SV = 9 at L = 4096).
 template <int SV>
 __global__ void __launch_bounds__(NT, 1)
-fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
+fft_correlate_kernel(int64_t T, int32_t L, int family, const uint64_t *__restrict__ phA,
                      const uint64_t *__restrict__ phB, const uint64_t *__restrict__ phC,
                      const float *__restrict__ inc2,
                      const float *__restrict__ ins2, const float2 *__restrict__ xspec,
@@ -81,7 +81,7 @@ fft_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         for (int s = 0; s < PTS; ++s) {
             const int n = t + NT * s;
             float sn = 0.0f, cs = 0.0f;
-            if (n < L) template_sincos(A, Bq, Cq, (uint32_t)n, &sn, &cs);
+            if (n < L) template_sincos(family, A, Bq, Cq, (uint32_t)n, &sn, &cs);
             G[s] = make_float2(cs, -sn);
         }
         fft8192(G, sm, t);
@@ -176,7 +176,7 @@ int launch_fft(const bfly_bank *b, const float *x, int64_t n_samples, int64_t la
     const int sv = (V + NT - 1) / NT;
 #define BFLY_FFT_LAUNCH(SV_)                                                                        \
     fft_correlate_kernel<SV_><<<(unsigned)ctas, NT, FFT_SMEM, stream>>>(                             \
-        b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->xspec, b->rn2, lag_begin, n_lags, V, \
+        b->T, b->L, b->family, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->xspec, b->rn2, lag_begin, n_lags, V, \
         (int32_t)n_blocks, rho_max, arg_lag)
     if (sv <= 9) BFLY_FFT_LAUNCH(9);
     else if (sv <= 13) BFLY_FFT_LAUNCH(13);

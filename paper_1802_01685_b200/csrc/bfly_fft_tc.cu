@@ -32,6 +32,13 @@ using namespace tc;
 #define BFLY_TC_HALF 0
 #endif
 constexpr bool TC_HALF = BFLY_TC_HALF != 0;
+
+// In-thread argmax of the block loop: 1 = compares in lag order (four values held back per
+// block), 2 = rank carried in the low mantissa bits + FMNMX3 tree, 0 = round-1 order (an exact
+// tie between lags l + 64 and l + 1 went to the larger lag).  Measured at config 4: see DESIGN.md.
+#ifndef BFLY_TC_EPI
+#define BFLY_TC_EPI 1
+#endif
 typedef ConstsT<TC_HALF> Consts;
 
 // ------------------------------------------------------------------------------------------
@@ -281,7 +288,9 @@ struct TailArgs {
     unsigned long long *n_hits;
 };
 
-template <bool TAILS, bool CUBIC>
+// FAM: 0 = linear chirps (32-bit phase arithmetic), 1 = cubic phase (reading N1, 64-bit Horner),
+// 2 = exponentially settling chirps (reading N2: phB / phC carry the doubles D tc and 1/(fs tc)).
+template <bool TAILS, int FAM>
 __global__ void __launch_bounds__(NT, 1)
 tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const uint64_t *__restrict__ phB, const uint64_t *__restrict__ phC,
@@ -340,28 +349,37 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         // ---- A3: synthesise g[n] = cos phi_n - i r sin phi_n, r = ||cos phi|| / ||sin phi||,
         //      n = 1024 a + 128 g + 16 c + d' < L, as the operand fragments of pass A (so that
         //      |z|^2 / ||cos phi||^2 is the quadrature sum); direct sums for the tail lags
-        const uint64_t A = phA[j], Bq = phB[j], Cq = CUBIC ? phC[j] : 0ull;
+        const uint64_t A = phA[j], Bq = phB[j], Cq = FAM != 0 ? phC[j] : 0ull;
         const uint32_t Ahi = (uint32_t)(A >> 32), Alo = (uint32_t)A;
         const uint32_t Bhi = (uint32_t)(Bq >> 32), Blo = (uint32_t)Bq;
         const float ic = inc2[j], rq = sqrtf(ins2[j] / ic);   // ic > 0: cos phi_0 = 1
         {
+            // The samples n >= 4096 are zero padding, so only the lanes t < 2 own non-zero operand
+            // words; the work is split over all four lanes of a group: lane t synthesises, for the
+            // owner lane t & 1, the units u = 4 (t >> 1) .. + 3, and the owners fetch the upper
+            // four units from lane + 2 by shuffle.
             uint32_t yr[8], yi[8];
             float tc_[MAX_TAIL], ts_[MAX_TAIL];
 #pragma unroll
             for (int r = 0; r < MAX_TAIL; ++r) tc_[r] = ts_[r] = 0.0f;
+            const int to = t & 1, uh = t >> 1;
+            uint32_t pr[4], pi[4];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int c = 4 * (w >> 3) + (u >> 1), dp = (w & 7) + 8 * (u & 1);
+            for (int kk = 0; kk < 4; ++kk) {
+                const int c = 4 * (w >> 3) + 2 * uh + (kk >> 1), dp = (w & 7) + 8 * (kk & 1);
                 float cs[2], sn[2];
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
-                    const int n = 1024 * (2 * t + e) + 128 * g + 16 * c + dp;
+                    const int n = 1024 * (2 * to + e) + 128 * g + 16 * c + dp;
                     cs[e] = sn[e] = 0.0f;
                     if (n < L) {
-                        if (!CUBIC) {                // linear chirp
+                        if (FAM == 0) {              // linear chirp
                             synth_sincos(Ahi, Alo, Bhi, Blo, (uint32_t)n, &sn[e], &cs[e]);
-                        } else {                     // reading N1: cubic phase, full 64-bit Horner
-                            const uint32_t ph = (uint32_t)(template_phase(A, Bq, Cq, (uint64_t)n) >> 32);
+                        } else {                     // N1: cubic phase, full 64-bit Horner; N2: settling
+                            const uint64_t p64 = FAM == 1 ? template_phase(A, Bq, Cq, (uint64_t)n)
+                                                          : settle_phase(A, __longlong_as_double((long long)Bq),
+                                                                         __longlong_as_double((long long)Cq), (uint64_t)n);
+                            const uint32_t ph = (uint32_t)(p64 >> 32);
                             const float ang = (float)(int32_t)ph * 1.4629180792671596e-9f;
                             sn[e] = __sinf(ang);
                             cs[e] = __cosf(ang);
@@ -382,8 +400,18 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                         }
                     }
                 }
-                yr[u] = pack_h2(cs[0], cs[1]);
-                yi[u] = pack_h2(-sn[0], -sn[1]);
+                pr[kk] = pack_h2(cs[0], cs[1]);
+                pi[kk] = pack_h2(-sn[0], -sn[1]);
+            }
+            const bool owner = t < 2;
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+                const uint32_t ur = __shfl_down_sync(0xffffffffu, pr[kk], 2);
+                const uint32_t ui = __shfl_down_sync(0xffffffffu, pi[kk], 2);
+                yr[kk] = owner ? pr[kk] : 0u;
+                yi[kk] = owner ? pi[kk] : 0u;
+                yr[4 + kk] = owner ? ur : 0u;
+                yi[4 + kk] = owner ? ui : 0u;
             }
             if (n_tail > 0) {
 #pragma unroll
@@ -410,23 +438,30 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             for (int h = 0; h < 2; ++h)
 #pragma unroll
                 for (int q = 0; q < 3; ++q) w16u[h][q] = sm.w16u[(h * 3 + q) * 32 + lane];
-            __half *gh = reinterpret_cast<__half *>(sm.gs);
-            const float r16 = 1.0f / S16;
+            // output m = U + 64 (2t + e) + 512 g + 4096 up (U = 4w + i) lives in operand_slot(m):
+            // thread ((e 8 + (U & 7)) 32 + (t + 4 (g & 1)) 4 + (g >> 2) + 2 up), word pair
+            // (U >> 3) & 1 of chunk U >> 4, half (g >> 1) & 1.  The lanes g and g ^ 2 hold the two
+            // halves of the same words: they exchange by shuffle, the lane with bit 1 of g clear
+            // writes the e = 0 words, the other the e = 1 words, {Re, Im} as one 8-byte store.
+            uint32_t *gw = reinterpret_cast<uint32_t *>(sm.gs);
+            const float2 r16 = make_float2(1.0f / S16, 1.0f / S16);
+            const int gb1 = (g >> 1) & 1;
+            const uint32_t sel = gb1 ? 0x3276u : 0x5410u;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 cpair z, zu;
                 chain2<true, TC_HALF>(k, sm.exch + wb * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, w16u);
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int m = (4 * w + i) + 64 * (2 * t + e) + 512 * g;
-                    int word, half;
-                    operand_slot(m, word, half);
-                    gh[2 * word + half] = __float2half_rn((e ? z.r.y : z.r.x) * r16);
-                    gh[2 * (word + 1) + half] = __float2half_rn((e ? z.i.y : z.i.x) * r16);
-                    operand_slot(m + 4096, word, half);
-                    gh[2 * word + half] = __float2half_rn((e ? zu.r.y : zu.r.x) * r16);
-                    gh[2 * (word + 1) + half] = __float2half_rn((e ? zu.i.y : zu.i.x) * r16);
-                }
+                const int U = 4 * w + i;
+                const float2 a0 = __fmul2_rn(z.r, r16), b0 = __fmul2_rn(z.i, r16);
+                const float2 a1 = __fmul2_rn(zu.r, r16), b1 = __fmul2_rn(zu.i, r16);
+                const uint32_t R0 = pack_h2(a0.x, a0.y), I0 = pack_h2(b0.x, b0.y);     // (e = 0, e = 1)
+                const uint32_t R1 = pack_h2(a1.x, a1.y), I1 = pack_h2(b1.x, b1.y);
+                const uint32_t oR0 = __shfl_xor_sync(0xffffffffu, R0, 8), oI0 = __shfl_xor_sync(0xffffffffu, I0, 8);
+                const uint32_t oR1 = __shfl_xor_sync(0xffffffffu, R1, 8), oI1 = __shfl_xor_sync(0xffffffffu, I1, 8);
+                const int tid0 = (gb1 * 8 + (U & 7)) * 32 + (t + 4 * (g & 1)) * 4 + (g >> 2);
+                const int word0 = ((U >> 4) * NT + tid0) * 4 + ((U >> 3) & 1) * 2;
+                *reinterpret_cast<uint2 *>(gw + word0) = make_uint2(__byte_perm(R0, oR0, sel), __byte_perm(I0, oI0, sel));
+                *reinterpret_cast<uint2 *>(gw + word0 + 8) = make_uint2(__byte_perm(R1, oR1, sel), __byte_perm(I1, oI1, sel));
             }
         }
         __syncthreads();
@@ -520,10 +555,43 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     qs4[i] = q;
                     qmax = fmaxf(qmax, fmaxf(q.x, q.y));
                 } else {
-                    if (q.x > best) { best = q.x; code = 8 * b + 2 * i; }
-                    if (q.y > best) { best = q.y; code = 8 * b + 2 * i + 1; }
+#if BFLY_TC_EPI == 2
+                    // A7 inside the thread: the low three mantissa bits of q (2^-21 relative, far
+                    // below the fp16 operand noise) carry 7 - (rank of the lag among the thread's
+                    // eight lags of this block: lag = .. + i + 64 e, so rank = 4 e + i): the
+                    // largest key is the largest q and, on a tie, the smallest lag (reading C8).
+                    // NaN (0 x -inf past the last lag) and -inf keys never win a maximum.
+                    qs4[i].x = __uint_as_float((__float_as_uint(q.x) & 0xFFFFFFF8u) | (uint32_t)(7 - i));
+                    qs4[i].y = __uint_as_float((__float_as_uint(q.y) & 0xFFFFFFF8u) | (uint32_t)(3 - i));
+#elif BFLY_TC_EPI == 1
+                    // A7 inside the thread, in lag order (reading C8: ties to the smallest lag): the
+                    // thread's lags of this block are .. + i + 64 e, so the e = 0 lags are compared
+                    // here and the e = 1 lags after the loop; code = 8 b + 4 e + i
+                    if (q.x > best) { best = q.x; code = 8 * b + i; }
+                    qs4[i].y = q.y;
+#else
+                    if (q.x > best) { best = q.x; code = 8 * b + i; }
+                    if (q.y > best) { best = q.y; code = 8 * b + 4 + i; }
+#endif
                 }
             }
+#if BFLY_TC_EPI == 2
+            if (!TAILS) {
+                const float bm = fmaxf(fmaxf(fmaxf(qs4[0].x, qs4[1].x), fmaxf(qs4[2].x, qs4[3].x)),
+                                       fmaxf(fmaxf(qs4[0].y, qs4[1].y), fmaxf(qs4[2].y, qs4[3].y)));
+                // `best` keeps its low bits at 7, so a later block wins only with a larger q
+                if (bm > best) {
+                    best = __uint_as_float(__float_as_uint(bm) | 7u);
+                    code = 8 * b + 7 - (int32_t)(__float_as_uint(bm) & 7u);
+                }
+            }
+#elif BFLY_TC_EPI == 1
+            if (!TAILS) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    if (qs4[i].y > best) { best = qs4[i].y; code = 8 * b + 4 + i; }
+            }
+#endif
             if (TAILS && qmax > thr) {                 // rare: at least one of this thread's 8 lags is a hit
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
@@ -561,7 +629,12 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 }
             } else {
                 const float q = fmaf(s, s, c * c) * __ldg(rn2 + (int64_t)n_blocks * TCV + tid);
+#if BFLY_TC_EPI == 2
+                const float qt = __uint_as_float(__float_as_uint(q) & 0xFFFFFFF8u);
+                if (qt > best) { best = __uint_as_float(__float_as_uint(qt) | 7u); code = 8 * n_blocks + tid; }
+#else
                 if (q > best) { best = q; code = 8 * n_blocks + tid; }
+#endif
             }
         }
         if (TAILS) {
@@ -569,12 +642,16 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             continue;
         }
         unsigned long long p = 0ull;
-        if (best > 0.0f) {
-            const int bb = code >> 3, sl = code & 7;
+        if (best > 0.0f) {                             // q = 0 everywhere: rho = 0 at the first lag, below
+            const int bb = code >> 3, rank = code & 7;            // rank = 4 e + i
             const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * TCV + (uint32_t)(code - 8 * n_blocks)
-                                               : (uint32_t)bb * TCV + (uint32_t)((4 * w + (sl >> 1)) +
-                                                                                 64 * (2 * t + (sl & 1)) + 512 * g);
+                                               : (uint32_t)bb * TCV + (uint32_t)((4 * w + (rank & 3)) +
+                                                                                 64 * (2 * t + (rank >> 2)) + 512 * g);
+#if BFLY_TC_EPI == 2
+            p = ((unsigned long long)(__float_as_uint(best) & 0xFFFFFFF8u) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
+#else
             p = ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
+#endif
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -660,10 +737,12 @@ static int tc_attrs(int device)
     return once.run(device, []() -> int {
         BFLY_CUDA(cudaFuncSetAttribute(tc_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_wspec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_debug_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         return BFLY_OK;
     });
@@ -696,17 +775,20 @@ static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_sample
     }
     const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
     core_timer_start(b, stream);
-#define BFLY_TC_LAUNCH(TAILS_, CUBIC_, ARGS_)                                                          \
-    tc_correlate_kernel<TAILS_, CUBIC_><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(                      \
+#define BFLY_TC_LAUNCH(TAILS_, FAM_, ARGS_)                                                            \
+    tc_correlate_kernel<TAILS_, FAM_><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(                        \
         b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh), \
         reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,    \
         rho_max, arg_lag, ARGS_)
+    const int fam = b->family == BFLY_FAMILY_SETTLE ? 2 : b->has_f2 ? 1 : 0;
     if (tails) {
-        if (b->has_f2) BFLY_TC_LAUNCH(true, true, *tails);
-        else BFLY_TC_LAUNCH(true, false, *tails);
+        if (fam == 2) BFLY_TC_LAUNCH(true, 2, *tails);
+        else if (fam == 1) BFLY_TC_LAUNCH(true, 1, *tails);
+        else BFLY_TC_LAUNCH(true, 0, *tails);
     } else {
-        if (b->has_f2) BFLY_TC_LAUNCH(false, true, TailArgs{});
-        else BFLY_TC_LAUNCH(false, false, TailArgs{});
+        if (fam == 2) BFLY_TC_LAUNCH(false, 2, TailArgs{});
+        else if (fam == 1) BFLY_TC_LAUNCH(false, 1, TailArgs{});
+        else BFLY_TC_LAUNCH(false, 0, TailArgs{});
     }
 #undef BFLY_TC_LAUNCH
     core_timer_stop(b, stream);

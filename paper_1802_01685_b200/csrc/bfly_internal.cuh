@@ -23,6 +23,11 @@ struct bfly_bank {
     uint64_t *phB;   // f1/(2 fs^2)      in units of 2^-64 cycles per sample^2
     uint64_t *phC;   // f2/(6 fs^3)      in units of 2^-64 cycles per sample^3
     int has_f2;      // some template has f2 != 0 (selects the cubic-phase kernel variants)
+    int family;      // BFLY_FAMILY_POLY: phA/phB/phC as above.  BFLY_FAMILY_SETTLE (reading N2):
+                     // f(t) = f_inf + D exp(-t/tc); phA = f_inf/fs as above, phB = the bits of the
+                     // double D tc [cycles], phC = the bits of the double 1/(fs tc) [1/sample];
+                     // f0/f1/f2 hold the frequency, slope and curvature at the first sample
+    double *s_finf, *s_delta, *s_tc;   // the settle family's own parameters (bfly_bank_get_settle)
     float *inc2;     // 1 / ||cos phi||^2 (0 if the norm is 0)
     float *ins2;     // 1 / ||sin phi||^2
     // workspace (grown by bfly_bank_reserve / on demand)
@@ -144,6 +149,7 @@ constexpr int FFT_MAX_L = FFT_B / 2;    // 4096
 
 // launchers (each enqueues on `stream`, returns a BFLY_* status)
 int launch_bank_params(bfly_bank *b, cudaStream_t stream);
+int launch_bank_params_settle(bfly_bank *b, cudaStream_t stream);
 int launch_sliding_norm(const float *x, int64_t n_samples, int32_t L, int64_t lag_begin,
                         int64_t n_lags, float *rn2, cudaStream_t stream);
 int launch_direct(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
@@ -182,10 +188,26 @@ __device__ __forceinline__ uint64_t template_phase(uint64_t A, uint64_t B, uint6
 {
     return ((C * k + B) * k + A) * k;
 }
-__device__ __forceinline__ void template_sincos(uint64_t A, uint64_t B, uint64_t C, uint32_t k, float *s,
-                                                float *c)
+// The settling family (reading N2): phi_k/2pi = f_inf k/fs + D tc (1 - exp(-k/(fs tc))).
+// The linear term is exact fixed point (A k mod 2^64); the exponential term is evaluated in float64
+// (-expm1 keeps full precision for k << fs tc; |D tc| of a few thousand cycles leaves an absolute
+// error of ~1e-12 cycle), reduced modulo one cycle and added as a 2^-64 fraction.
+__device__ __forceinline__ uint64_t settle_phase(uint64_t A, double Dtc, double inv_fstc, uint64_t k)
 {
-    uint64_t ph = template_phase(A, B, C, k);
+    double v = Dtc * (-expm1(-inv_fstc * (double)k));
+    v -= floor(v);                                           // [0, 1)
+    return A * k + __double2ull_rz(v * 18446744073709551616.0);
+}
+__device__ __forceinline__ uint64_t family_phase(int family, uint64_t A, uint64_t B, uint64_t C, uint64_t k)
+{
+    if (family == BFLY_FAMILY_SETTLE)
+        return settle_phase(A, __longlong_as_double((long long)B), __longlong_as_double((long long)C), k);
+    return template_phase(A, B, C, k);
+}
+__device__ __forceinline__ void template_sincos(int family, uint64_t A, uint64_t B, uint64_t C, uint32_t k,
+                                                float *s, float *c)
+{
+    uint64_t ph = family_phase(family, A, B, C, k);
     // top 32 bits as a signed fraction of a half-turn: angle = pi * v, v in [-1, 1)
     float v = (float)(int32_t)(uint32_t)(ph >> 32) * 4.656612873077393e-10f;  // 2^-31
     sincospif(v, s, c);

@@ -52,6 +52,10 @@ def test_argument_validation_happens_before_any_device_work():
     with pytest.raises(bfly.BflyError) as e:
         bfly.make_bank(-1.0, 4096, [100.0], [1.0])
     assert e.value.status == -1
+    for tc in (0.0, -1.0, np.inf, np.nan):                   # the settling family: tc finite and > 0
+        with pytest.raises(bfly.BflyError) as e:
+            bfly.make_bank_settle(4096.0, 4096, [1200.0], [300.0], [tc])
+        assert e.value.status == -1
 
 
 def test_no_cpu_fallback_without_a_device():
