@@ -188,7 +188,8 @@ struct TcSmem {
     float *xt;                 // x[first tail lag ..], L + MAX_TAIL - 1 samples at xt_slot(n) (direct tail lags)
     uint32_t *w16u;            // [2][3][32]: A fragments of W16 rows 8..15 (G transform only)
     float *tail;               // [16 warps][2 MAX_TAIL] partial sums of the direct tail lags
-    unsigned long long *red;   // [16]
+    unsigned long long *red;   // [2][16]
+    unsigned char *par;        // [2][32]: {phA, phB, phC, inc2, ins2} of the template after this one
     unsigned long long *bar;   // mbarriers: [0..2] exchange buffer full, [3..4] X_b slot filled
 };
 constexpr int N_EXCH = 3;
@@ -198,8 +199,9 @@ constexpr size_t OFF_XT = OFF_XS + 2 * EXCH_WORDS * 4;
 constexpr size_t OFF_W16U = OFF_XT + (FFT_MAX_L + 32) * 4;
 constexpr size_t OFF_TAIL = OFF_W16U + 2 * 3 * 32 * 4;
 constexpr size_t OFF_RED = OFF_TAIL + 16 * 2 * MAX_TAIL * 4;
-constexpr size_t OFF_BAR = OFF_RED + 16 * 8;
-constexpr size_t TC_SMEM = OFF_BAR + 8 * 8;
+constexpr size_t OFF_BAR = OFF_RED + 2 * 16 * 8;              // red[] is double buffered by template parity
+constexpr size_t OFF_PAR = OFF_BAR + 8 * 8;                   // two slots of prefetched bank parameters
+constexpr size_t TC_SMEM = OFF_PAR + 2 * 32;
 __device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
 {
     TcSmem s;
@@ -211,6 +213,7 @@ __device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
     s.tail = reinterpret_cast<float *>(base + OFF_TAIL);
     s.red = reinterpret_cast<unsigned long long *>(base + OFF_RED);
     s.bar = reinterpret_cast<unsigned long long *>(base + OFF_BAR);
+    s.par = base + OFF_PAR;
     return s;
 }
 
@@ -263,6 +266,17 @@ __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t b
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+
+// cp.async (LDGSTS) of 8 / 4 bytes: the bank parameters of the CTA's next template travel to shared
+// memory while the current template runs, so that no template starts with a DRAM round trip
+__device__ __forceinline__ void cp_async8(void *dst, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void *dst, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr(dst)), "l"(src) : "memory");
 }
 
 // One CTA per SM, persistent, strided over the bank; one template at a time.  Per template: g is
@@ -345,14 +359,42 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
     int wb = 0, rb = 0;                                // exchange buffer written next / read next
     uint32_t fpar = 0;                                 // bit i: parity to wait for on "full(i)"
 
-    for (int64_t j = blockIdx.x; j < T; j += gridDim.x) {
+    auto prefetch_params = [&](int64_t jn, int slot) {            // thread 0 only
+        unsigned char *d = sm.par + 32 * slot;
+        cp_async8(d, phA + jn);
+        cp_async8(d + 8, phB + jn);
+        if (FAM != 0) cp_async8(d + 16, phC + jn);
+        cp_async4(d + 24, inc2 + jn);
+        cp_async4(d + 28, ins2 + jn);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if (tid == 0 && blockIdx.x < T) {
+        prefetch_params(blockIdx.x, 0);
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+    int ps = 0;                                                  // parameter slot / red[] half of this template
+    for (int64_t j = blockIdx.x; j < T; j += gridDim.x, ps ^= 1) {
         // ---- A3: synthesise g[n] = cos phi_n - i r sin phi_n, r = ||cos phi|| / ||sin phi||,
         //      n = 1024 a + 128 g + 16 c + d' < L, as the operand fragments of pass A (so that
         //      |z|^2 / ||cos phi||^2 is the quadrature sum); direct sums for the tail lags
-        const uint64_t A = phA[j], Bq = phB[j], Cq = FAM != 0 ? phC[j] : 0ull;
+        const unsigned char *pp = sm.par + 32 * ps;
+        const uint64_t A = *reinterpret_cast<const uint64_t *>(pp), Bq = *reinterpret_cast<const uint64_t *>(pp + 8);
+        const uint64_t Cq = FAM != 0 ? *reinterpret_cast<const uint64_t *>(pp + 16) : 0ull;
         const uint32_t Ahi = (uint32_t)(A >> 32), Alo = (uint32_t)A;
         const uint32_t Bhi = (uint32_t)(Bq >> 32), Blo = (uint32_t)Bq;
-        const float ic = inc2[j], rq = sqrtf(ins2[j] / ic);   // ic > 0: cos phi_0 = 1
+        const float ic = *reinterpret_cast<const float *>(pp + 24);
+        const float rq = sqrtf(*reinterpret_cast<const float *>(pp + 28) / ic);   // ic > 0: cos phi_0 = 1
+        if (tid == 0 && j + gridDim.x < T) prefetch_params(j + gridDim.x, ps ^ 1);
+        // The index arithmetic of the per-template code below depends on the thread only, so the
+        // compiler would hoist it out of the template loop and hold its results in registers all
+        // through the block loop -- which is at the 128-register limit and then recomputes its OWN
+        // addresses on every block (measured: +24 instructions per block).  An opaque copy of the
+        // thread index keeps that arithmetic here, where it costs a few dozen cheap instructions
+        // per template.
+        int ptid = tid;
+        asm volatile("" : "+r"(ptid));
+        const int pl = ptid & 31, pw = ptid >> 5, pg = pl >> 2, pt = pl & 3;
         {
             // The samples n >= 4096 are zero padding, so only the lanes t < 2 own non-zero operand
             // words; the work is split over all four lanes of a group: lane t synthesises, for the
@@ -362,15 +404,15 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             float tc_[MAX_TAIL], ts_[MAX_TAIL];
 #pragma unroll
             for (int r = 0; r < MAX_TAIL; ++r) tc_[r] = ts_[r] = 0.0f;
-            const int to = t & 1, uh = t >> 1;
+            const int to = pt & 1, uh = pt >> 1;
             uint32_t pr[4], pi[4];
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
-                const int c = 4 * (w >> 3) + 2 * uh + (kk >> 1), dp = (w & 7) + 8 * (kk & 1);
+                const int c = 4 * (pw >> 3) + 2 * uh + (kk >> 1), dp = (pw & 7) + 8 * (kk & 1);
                 float cs[2], sn[2];
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
-                    const int n = 1024 * (2 * to + e) + 128 * g + 16 * c + dp;
+                    const int n = 1024 * (2 * to + e) + 128 * pg + 16 * c + dp;
                     cs[e] = sn[e] = 0.0f;
                     if (n < L) {
                         if (FAM == 0) {              // linear chirp
@@ -403,7 +445,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 pr[kk] = pack_h2(cs[0], cs[1]);
                 pi[kk] = pack_h2(-sn[0], -sn[1]);
             }
-            const bool owner = t < 2;
+            const bool owner = pt < 2;
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
                 const uint32_t ur = __shfl_down_sync(0xffffffffu, pr[kk], 2);
@@ -422,9 +464,9 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                         tc_[r] += __shfl_xor_sync(0xffffffffu, tc_[r], o);
                         ts_[r] += __shfl_xor_sync(0xffffffffu, ts_[r], o);
                     }
-                    if (lane == 0) {
-                        sm.tail[(w * MAX_TAIL + r) * 2] = tc_[r];
-                        sm.tail[(w * MAX_TAIL + r) * 2 + 1] = ts_[r];
+                    if (pl == 0) {
+                        sm.tail[(pw * MAX_TAIL + r) * 2] = tc_[r];
+                        sm.tail[(pw * MAX_TAIL + r) * 2 + 1] = ts_[r];
                     }
                 }
             }
@@ -445,20 +487,20 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             // writes the e = 0 words, the other the e = 1 words, {Re, Im} as one 8-byte store.
             uint32_t *gw = reinterpret_cast<uint32_t *>(sm.gs);
             const float2 r16 = make_float2(1.0f / S16, 1.0f / S16);
-            const int gb1 = (g >> 1) & 1;
+            const int gb1 = (pg >> 1) & 1;
             const uint32_t sel = gb1 ? 0x3276u : 0x5410u;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 cpair z, zu;
                 chain2<true, TC_HALF>(k, sm.exch + wb * (EXCH_WORDS / 4), 4 * w + i, lane, z, zu, w16u);
-                const int U = 4 * w + i;
+                const int U = 4 * pw + i;
                 const float2 a0 = __fmul2_rn(z.r, r16), b0 = __fmul2_rn(z.i, r16);
                 const float2 a1 = __fmul2_rn(zu.r, r16), b1 = __fmul2_rn(zu.i, r16);
                 const uint32_t R0 = pack_h2(a0.x, a0.y), I0 = pack_h2(b0.x, b0.y);     // (e = 0, e = 1)
                 const uint32_t R1 = pack_h2(a1.x, a1.y), I1 = pack_h2(b1.x, b1.y);
                 const uint32_t oR0 = __shfl_xor_sync(0xffffffffu, R0, 8), oI0 = __shfl_xor_sync(0xffffffffu, I0, 8);
                 const uint32_t oR1 = __shfl_xor_sync(0xffffffffu, R1, 8), oI1 = __shfl_xor_sync(0xffffffffu, I1, 8);
-                const int tid0 = (gb1 * 8 + (U & 7)) * 32 + (t + 4 * (g & 1)) * 4 + (g >> 2);
+                const int tid0 = (gb1 * 8 + (U & 7)) * 32 + (pt + 4 * (pg & 1)) * 4 + (pg >> 2);
                 const int word0 = ((U >> 4) * NT + tid0) * 4 + ((U >> 3) & 1) * 2;
                 *reinterpret_cast<uint2 *>(gw + word0) = make_uint2(__byte_perm(R0, oR0, sel), __byte_perm(I0, oI0, sel));
                 *reinterpret_cast<uint2 *>(gw + word0 + 8) = make_uint2(__byte_perm(R1, oR1, sel), __byte_perm(I1, oI1, sel));
@@ -637,6 +679,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 #endif
             }
         }
+        if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");   // the next template's parameters
         if (TAILS) {
             __syncthreads();                            // red[], tail[], gs, exch are reused by the next template
             continue;
@@ -658,11 +701,12 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             const unsigned long long q = __shfl_xor_sync(0xffffffffu, p, o);
             p = q > p ? q : p;
         }
-        if (lane == 0) sm.red[w] = p;
-        __syncthreads();
-        if (tid == 0) {
+        unsigned long long *red = sm.red + 16 * ps;
+        if (lane == 0) red[w] = p;
+        __syncthreads();                                // also: every warp is done with gs, exch, tail[]
+        if (tid == 0) {                                 // the other threads go on to the next template
 #pragma unroll
-            for (int ww = 1; ww < 16; ++ww) p = sm.red[ww] > p ? sm.red[ww] : p;
+            for (int ww = 1; ww < 16; ++ww) p = red[ww] > p ? red[ww] : p;
             if (p == 0ull) {                            // rho = 0 at every lag (or no lag at all)
                 rho_max[j] = 0.0f;
                 arg_lag[j] = (int32_t)lag_begin;
@@ -671,7 +715,6 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 arg_lag[j] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
             }
         }
-        __syncthreads();                                // red[], tail[], gs, exch are reused by the next template
     }
 }
 

@@ -136,3 +136,49 @@ def test_tails_lag_subrange_scale_and_edges(bfly):
         _tails(bfly, 512.0, 64, [50.0], [1.0], x, 3.5, 16)
     with pytest.raises(bfly.BflyError):                       # kappa must be > 0
         _tails(bfly, fs, L, f0, f1, x, 0.0, 16)
+
+
+def test_tails_full_bank_config4_sampled_against_the_oracle(bfly):
+    """bfly_tails over BASELINE.json's paper-scale bank (2^23 templates x 61441 lags, kappa = 5.5:
+    ~1.5e5 hits, the launch bench.py times): the hit list of sampled templates -- half of them
+    drawn from the templates that have hits, half from those that have none -- against the oracle
+    (R5), sigma included; no duplicate (template, lag) in the whole list; a sub-bank run of the same
+    templates gives the same sigmas and hits bit for bit (R4)."""
+    cfg = get_config(4)
+    x = make_data(cfg)
+    xd = torch.from_numpy(x).cuda()
+    full = bfly.make_bank_grid(cfg.fs_hz, cfg.L, cfg.f0_lo, cfg.f0_hi, cfg.n_f0, cfg.f1_lo, cfg.f1_hi, cfg.n_f1)
+    kappa, cap = 5.5, 1 << 22
+    sig, hj, hl, hr, n = bfly.tails(full, xd, kappa, cap)
+    torch.cuda.synchronize()
+    total = int(n.item())
+    assert 0 < total < cap
+    hj_n, hl_n, hr_n = hj.cpu().numpy()[:total], hl.cpu().numpy()[:total], hr.cpu().numpy()[:total]
+    key = hj_n.astype(np.int64) * (1 << 20) + hl_n
+    assert len(np.unique(key)) == total                      # no duplicates anywhere
+    assert np.all((hl_n >= 0) & (hl_n < cfg.n_lags)) and np.all(hr_n > kappa)
+    rng = np.random.default_rng(44)
+    with_hits = np.unique(hj_n)
+    mask = np.ones(len(full), bool)
+    mask[with_hits] = False
+    without = np.nonzero(mask)[0]
+    idx = np.sort(np.concatenate([rng.choice(with_hits, 60, replace=False), rng.choice(without, 60, replace=False),
+                                  [0, len(full) - 1]]))
+    idx = np.unique(idx)
+    f0a, f1a = bank_grid(cfg)
+    pos = {int(j): i for i, j in enumerate(idx)}
+    sel = np.isin(hj_n, idx)
+    sub_j = np.array([pos[int(j)] for j in hj_n[sel]], np.int32)
+    sig_n = sig.cpu().numpy()
+    n_or, n_border = check_tails(x, cfg.fs_hz, cfg.L, f0a[idx], f1a[idx], kappa, sig_n[idx], sub_j, hl_n[sel],
+                                 hr_n[sel], int(sel.sum()))
+    print(f"tails, config 4 full bank: {total} hits; {len(idx)} sampled templates: {int(sel.sum())} gpu hits, "
+          f"{n_or} oracle hits, {n_border} within tolerance of kappa")
+    sub = bfly.make_bank(cfg.fs_hz, cfg.L, f0a[idx], f1a[idx])
+    sig2, hj2, hl2, hr2, n2 = bfly.tails(sub, xd, kappa, 1 << 16)
+    torch.cuda.synchronize()
+    t2 = int(n2.item())
+    assert np.array_equal(sig2.cpu().numpy(), sig_n[idx]) and t2 == int(sel.sum())
+    a = sorted(zip(sub_j.tolist(), hl_n[sel].tolist(), hr_n[sel].tolist()))
+    b = sorted(zip(hj2.cpu().numpy()[:t2].tolist(), hl2.cpu().numpy()[:t2].tolist(), hr2.cpu().numpy()[:t2].tolist()))
+    assert a == b
