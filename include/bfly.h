@@ -281,6 +281,15 @@ int bfly_bank_core_ms(bfly_bank *bank, float *ms_out);
  * |y| must stay within the fp16 range.  Asynchronous on `stream`. */
 int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream);
 
+/* Diagnostic (tests and DESIGN.md 10 only): the same transform on the 5th-generation tensor cores
+ * (tcgen05.mma kind::f16, DFT matrices resident in tensor memory, data through swizzled shared
+ * memory; csrc/bfly_fft_tc5.cu), outputs n < 4096 only.  y_dev: DEVICE, 2 n_pairs transforms of
+ * 8192 interleaved complex fp32; z_dev: DEVICE, 2 n_pairs x 4096 interleaved complex fp32,
+ * overwritten.  One CTA; `reps` repeats every pair (timing: cycles_dev[0], optional DEVICE int64,
+ * receives the SM clock cycles of the whole loop).  Asynchronous on `stream`. */
+int bfly_debug_fft_tc5(const float *y_dev, float *z_dev, int32_t n_pairs, int32_t reps, int64_t *cycles_dev,
+                       void *stream);
+
 /* Measurement aid (bench.py's roofline denominators; "measured by a microbenchmark
  * on the box"): runs one microbenchmark kernel on every SM of the CURRENT device (two warm-up
  * launches, the third timed with CUDA events) and returns its rate.  Synchronous.
@@ -295,7 +304,8 @@ int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream);
  *                    memory, 2 = A from tensor memory, 0 = none; bit 2: N = 256 instead of 128),
  *                    [1] = clocks per iteration of 16 warps streaming beside it (bit 3: 32 KB of
  *                    st.shared.v4 + 32 KB of ld.shared.v4 per iteration; bit 4: 64 KB of
- *                    tcgen05.ld per iteration)
+ *                    tcgen05.ld per iteration; bit 5: consecutive MMAs accumulate into two tiles
+ *                    in turn; bit 6: N = 64)
  * `variant` is ignored by the others.  ms_out (optional): the timed launch in milliseconds. */
 enum { BFLY_PEAK_FFMA = 0, BFLY_PEAK_FFMA2 = 1, BFLY_PEAK_LDS = 2, BFLY_PEAK_HMMA = 3,
        BFLY_PEAK_SHFL = 4, BFLY_PEAK_L2 = 5, BFLY_PEAK_UMMA = 6 };

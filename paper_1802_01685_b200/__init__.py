@@ -18,7 +18,7 @@ from . import build as _build
 __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
            "butterfly_map", "search_host", "launch_count", "lib_path",
            "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC",
-           "debug_fft_tc", "tails", "hits_map", "time_randomize", "coincidence", "pseudo_spectrum",
+           "debug_fft_tc", "debug_fft_tc5", "tails", "hits_map", "time_randomize", "coincidence", "pseudo_spectrum",
            "make_bank_settle", "FAMILY_POLY", "FAMILY_SETTLE", "debug_peak", "PEAK_FFMA", "PEAK_FFMA2", "PEAK_LDS", "PEAK_HMMA", "PEAK_SHFL", "PEAK_L2",
            "PEAK_UMMA"]
 
@@ -71,12 +71,13 @@ def _load():
     lib.bfly_bank_set_timing.argtypes = [vp, C.c_int]
     lib.bfly_bank_core_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.bfly_debug_fft_tc.argtypes = [vp, vp, C.c_int, vp]
+    lib.bfly_debug_fft_tc5.argtypes = [vp, vp, i32, i32, vp, vp]
     lib.bfly_debug_peak.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(f64), C.POINTER(f64)]
     lib.bfly_launch_count.argtypes = []
     lib.bfly_launch_count.restype = i64
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
                  "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
-                 "bfly_search_host", "bfly_debug_fft_tc", "bfly_tails", "bfly_hits_map",
+                 "bfly_search_host", "bfly_debug_fft_tc", "bfly_debug_fft_tc5", "bfly_tails", "bfly_hits_map",
                  "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum",
                  "bfly_make_bank3", "bfly_bank_get_f2", "bfly_debug_peak", "bfly_make_bank_settle",
                  "bfly_bank_get_settle", "bfly_bank_family"):
@@ -403,6 +404,20 @@ def debug_peak(which: int, variant: int = 0, iters: int = 2000, device: int = 0)
         _check(_lib.bfly_debug_peak(int(which), int(variant), int(iters), out, C.byref(ms)),
                "bfly_debug_peak")
     return ((out[0], out[1]) if which == PEAK_UMMA else out[0]), ms.value
+
+
+def debug_fft_tc5(y: torch.Tensor, reps: int = 1):
+    """bfly_debug_fft_tc5: the length-8192 transform on tcgen05 for complex64[2 p, 8192] device
+    input (tests only).  Returns (complex64[2 p, 4096], SM clock cycles of the whole loop)."""
+    if y.dtype != torch.complex64 or y.dim() != 2 or y.shape[1] != 8192 or y.shape[0] % 2 or not y.is_cuda \
+            or not y.is_contiguous():
+        raise TypeError("y must be a contiguous complex64[2 p, 8192] CUDA tensor")
+    z = torch.zeros((y.shape[0], 4096), dtype=torch.complex64, device=y.device)
+    cyc = torch.zeros(1, dtype=torch.int64, device=y.device)
+    _check(_lib.bfly_debug_fft_tc5(C.c_void_p(y.data_ptr()), C.c_void_p(z.data_ptr()), y.shape[0] // 2,
+                                   int(reps), C.c_void_p(cyc.data_ptr()), _stream(y.device.index)),
+           "bfly_debug_fft_tc5")
+    return z, cyc
 
 
 def launch_count() -> int:

@@ -529,6 +529,17 @@ int bfly_debug_fft_tc(const float *y_dev, float *z_dev, int full, void *stream)
                                reinterpret_cast<float2 *>(z_dev), full, (cudaStream_t)stream);
 }
 
+int bfly_debug_fft_tc5(const float *y_dev, float *z_dev, int32_t n_pairs, int32_t reps, int64_t *cycles_dev,
+                       void *stream)
+{
+    if (!y_dev || !z_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n_pairs < 1 || reps < 1) { set_error("n_pairs and reps must be >= 1"); return BFLY_EINVAL; }
+    int rc = current_device_ok();
+    if (rc) return rc;
+    return launch_debug_fft_tc5(reinterpret_cast<const float2 *>(y_dev), reinterpret_cast<float2 *>(z_dev),
+                                n_pairs, reps, reinterpret_cast<long long *>(cycles_dev), (cudaStream_t)stream);
+}
+
 int bfly_correlate(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int64_t lag_begin,
                    int64_t lag_end, float *rho_max_dev, int32_t *arg_lag_dev, void *stream)
 {

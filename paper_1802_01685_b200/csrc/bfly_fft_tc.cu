@@ -39,6 +39,13 @@ constexpr bool TC_HALF = BFLY_TC_HALF != 0;
 #ifndef BFLY_TC_EPI
 #define BFLY_TC_EPI 1
 #endif
+// Half of the warps of every scheduler run the two halves of a block iteration in the other order.
+#ifndef BFLY_TC_PEEL
+#define BFLY_TC_PEEL 0
+#endif
+#ifndef BFLY_TC_DEPHASE
+#define BFLY_TC_DEPHASE 0
+#endif
 typedef ConstsT<TC_HALF> Consts;
 
 // ------------------------------------------------------------------------------------------
@@ -580,76 +587,101 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             }
             const uint4 *rbuf = sm.exch + rb * (EXCH_WORDS / 4);
             rb = rb + 1 == N_EXCH ? 0 : rb + 1;
-            if (b + 1 < n_blocks) front();
-            // ---- passes C, D and A5-A7 on the 8 lags of this thread
-            const float4 *rp = rn2p + ((int64_t)b * NT + tid) * 2;
-            const float4 ra = __ldg(rp), rb4 = __ldg(rp + 1);
-            const float2 rr[4] = {make_float2(ra.x, ra.y), make_float2(ra.z, ra.w),
-                                  make_float2(rb4.x, rb4.y), make_float2(rb4.z, rb4.w)};
-            float2 qs4[4];
-            float qmax = 0.0f;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                cpair z, zu;
-                chain2<false, TC_HALF>(k, rbuf, 4 * w + i, lane, z, zu, nowu);
-                const float2 q = __fmul2_rn(__ffma2_rn(z.i, z.i, __fmul2_rn(z.r, z.r)), rr[i]);
-                if (TAILS) {
-                    qs4[i] = q;
-                    qmax = fmaxf(qmax, fmaxf(q.x, q.y));
-                } else {
-#if BFLY_TC_EPI == 2
-                    // A7 inside the thread: the low three mantissa bits of q (2^-21 relative, far
-                    // below the fp16 operand noise) carry 7 - (rank of the lag among the thread's
-                    // eight lags of this block: lag = .. + i + 64 e, so rank = 4 e + i): the
-                    // largest key is the largest q and, on a tie, the smallest lag (reading C8).
-                    // NaN (0 x -inf past the last lag) and -inf keys never win a maximum.
-                    qs4[i].x = __uint_as_float((__float_as_uint(q.x) & 0xFFFFFFF8u) | (uint32_t)(7 - i));
-                    qs4[i].y = __uint_as_float((__float_as_uint(q.y) & 0xFFFFFFF8u) | (uint32_t)(3 - i));
-#elif BFLY_TC_EPI == 1
-                    // A7 inside the thread, in lag order (reading C8: ties to the smallest lag): the
-                    // thread's lags of this block are .. + i + 64 e, so the e = 0 lags are compared
-                    // here and the e = 1 lags after the loop; code = 8 b + 4 e + i
-                    if (q.x > best) { best = q.x; code = 8 * b + i; }
-                    qs4[i].y = q.y;
-#else
-                    if (q.x > best) { best = q.x; code = 8 * b + i; }
-                    if (q.y > best) { best = q.y; code = 8 * b + 4 + i; }
-#endif
-                }
-            }
-#if BFLY_TC_EPI == 2
-            if (!TAILS) {
-                const float bm = fmaxf(fmaxf(fmaxf(qs4[0].x, qs4[1].x), fmaxf(qs4[2].x, qs4[3].x)),
-                                       fmaxf(fmaxf(qs4[0].y, qs4[1].y), fmaxf(qs4[2].y, qs4[3].y)));
-                // `best` keeps its low bits at 7, so a later block wins only with a larger q
-                if (bm > best) {
-                    best = __uint_as_float(__float_as_uint(bm) | 7u);
-                    code = 8 * b + 7 - (int32_t)(__float_as_uint(bm) & 7u);
-                }
-            }
-#elif BFLY_TC_EPI == 1
-            if (!TAILS) {
-#pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    if (qs4[i].y > best) { best = qs4[i].y; code = 8 * b + 4 + i; }
-            }
-#endif
-            if (TAILS && qmax > thr) {                 // rare: at least one of this thread's 8 lags is a hit
+            // ---- the two halves of an iteration, passes A, B of block b + 1 ("front") and passes C, D
+            //      + A5-A7 of block b ("back"), are independent; half of the warps of every scheduler
+            //      (w >> 3) run them in the other order, so that the tensor-pipe bursts of one half
+            //      fall on the FMA / ALU bursts of the other (measured: DESIGN.md 10)
+            auto back = [&]() {
+                // ---- passes C, D and A5-A7 on the 8 lags of this thread
+                const float4 *rp = rn2p + ((int64_t)b * NT + tid) * 2;
+                const float4 ra = __ldg(rp), rb4 = __ldg(rp + 1);
+                const float2 rr[4] = {make_float2(ra.x, ra.y), make_float2(ra.z, ra.w),
+                                      make_float2(rb4.x, rb4.y), make_float2(rb4.z, rb4.w)};
+                float2 qs4[4];
+                float qmax = 0.0f;
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
+                    cpair z, zu;
+                    chain2<false, TC_HALF>(k, rbuf, 4 * w + i, lane, z, zu, nowu);
+                    const float2 q = __fmul2_rn(__ffma2_rn(z.i, z.i, __fmul2_rn(z.r, z.r)), rr[i]);
+                    if (TAILS) {
+                        qs4[i] = q;
+                        qmax = fmaxf(qmax, fmaxf(q.x, q.y));
+                    } else {
+#if BFLY_TC_EPI == 2
+                        // A7 inside the thread: the low three mantissa bits of q (2^-21 relative, far
+                        // below the fp16 operand noise) carry 7 - (rank of the lag among the thread's
+                        // eight lags of this block: lag = .. + i + 64 e, so rank = 4 e + i): the
+                        // largest key is the largest q and, on a tie, the smallest lag (reading C8).
+                        // NaN (0 x -inf past the last lag) and -inf keys never win a maximum.
+                        qs4[i].x = __uint_as_float((__float_as_uint(q.x) & 0xFFFFFFF8u) | (uint32_t)(7 - i));
+                        qs4[i].y = __uint_as_float((__float_as_uint(q.y) & 0xFFFFFFF8u) | (uint32_t)(3 - i));
+#elif BFLY_TC_EPI == 1
+                        // A7 inside the thread, in lag order (reading C8: ties to the smallest lag): the
+                        // thread's lags of this block are .. + i + 64 e, so the e = 0 lags are compared
+                        // here and the e = 1 lags after the loop; code = 8 b + 4 e + i
+                        if (q.x > best) { best = q.x; code = 8 * b + i; }
+                        qs4[i].y = q.y;
+#else
+                        if (q.x > best) { best = q.x; code = 8 * b + i; }
+                        if (q.y > best) { best = q.y; code = 8 * b + 4 + i; }
+#endif
+                    }
+                }
+#if BFLY_TC_EPI == 2
+                if (!TAILS) {
+                    const float bm = fmaxf(fmaxf(fmaxf(qs4[0].x, qs4[1].x), fmaxf(qs4[2].x, qs4[3].x)),
+                                           fmaxf(fmaxf(qs4[0].y, qs4[1].y), fmaxf(qs4[2].y, qs4[3].y)));
+                    // `best` keeps its low bits at 7, so a later block wins only with a larger q
+                    if (bm > best) {
+                        best = __uint_as_float(__float_as_uint(bm) | 7u);
+                        code = 8 * b + 7 - (int32_t)(__float_as_uint(bm) & 7u);
+                    }
+                }
+#elif BFLY_TC_EPI == 1
+                if (!TAILS) {
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const float qe = e ? qs4[i].y : qs4[i].x;
-                        if (qe > thr) {
-                            const unsigned long long at = atomicAdd(ta.n_hits, 1ull);
-                            if (at < (unsigned long long)ta.capacity) {
-                                ta.hit_template[at] = (int32_t)j;
-                                ta.hit_lag[at] = (int32_t)(lag_begin + (int64_t)b * TCV + (4 * w + i) + 64 * (2 * t + e) + 512 * g);
-                                ta.hit_rho[at] = sqrtf(qe * rsig2);
+                    for (int i = 0; i < 4; ++i)
+                        if (qs4[i].y > best) { best = qs4[i].y; code = 8 * b + 4 + i; }
+                }
+#endif
+                if (TAILS && qmax > thr) {                 // rare: at least one of this thread's 8 lags is a hit
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const float qe = e ? qs4[i].y : qs4[i].x;
+                            if (qe > thr) {
+                                const unsigned long long at = atomicAdd(ta.n_hits, 1ull);
+                                if (at < (unsigned long long)ta.capacity) {
+                                    ta.hit_template[at] = (int32_t)j;
+                                    ta.hit_lag[at] = (int32_t)(lag_begin + (int64_t)b * TCV + (4 * w + i) + 64 * (2 * t + e) + 512 * g);
+                                    ta.hit_rho[at] = sqrtf(qe * rsig2);
+                                }
                             }
                         }
                     }
                 }
+        
+            };
+#if BFLY_TC_DEPHASE
+            if (w & 8) {
+                back();
+                if (b + 1 < n_blocks) front();
+            } else
+#endif
+            {
+#if BFLY_TC_PEEL
+                if (b + 1 < n_blocks) {                // one straight-line stretch: the scheduler may interleave the two
+                    front();
+                    back();
+                } else {
+                    back();
+                }
+#else
+                if (b + 1 < n_blocks) front();
+                back();
+#endif
             }
         }
         // ---- tail lags (direct sums) and the CTA-wide maximum, ties to the smallest lag

@@ -181,6 +181,7 @@ int launch_pseudo_spectrum(const uint32_t *m, int32_t n_tbins, int32_t n_fbins,
 int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin, int64_t lag_end,
                     float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream);
+int launch_debug_fft_tc5(const float2 *y, float2 *z, int n_pairs, int reps, long long *cycles_dev, cudaStream_t stream);
 
 // Template phase in cycles, as a 64-bit fixed-point fraction:
 // phi_k/2pi mod 1 = (A k + B k^2 + C k^3) 2^-64 (Horner, modulo 2^64: the wrap is the mod 1).

@@ -138,6 +138,8 @@ __global__ void __launch_bounds__(512) peak_l2_kernel(const uint4 *__restrict__ 
 //               2  : N = 256 instead of 128
 //               3  : warps 0-15 stream st.shared.v4 + ld.shared.v4 over 64 KB
 //               4  : warps 0-15 stream tcgen05.ld.32x32b.x32
+//               5  : consecutive MMAs accumulate into two different tiles in turn (N <= 128)
+//               6  : N = 64
 // results[0] = clock cycles of the MMA thread, results[1] = cycles of the slowest streaming warp
 constexpr int PK_THREADS = 17 * 32;
 constexpr size_t PK_SMEM = 1024 + 32768 + 32768 + 65536 + 256;
@@ -176,15 +178,20 @@ __global__ void __launch_bounds__(PK_THREADS, 1) peak_umma_kernel(long long *cyc
     long long t0 = clock64();
     if (tid == 16 * 32) {
         if (mma_mode) {
-            const uint32_t idesc = idesc_f16(128, wide ? 256 : 128);
+            const int n_cols = (variant & 64) ? 64 : wide ? 256 : 128;
+            const bool interleave = variant & 32;     // consecutive MMAs accumulate into different tiles
+            const uint32_t idesc = idesc_f16(128, n_cols);
             const uint64_t da = smem_desc_k128(a_tile), db = smem_desc_k128(b_tile);
             for (int i = 0; i < iters; ++i) {
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
                     // four K-steps inside each of two 64-wide swizzle atoms of both tiles
                     const uint32_t ko = (uint32_t)(k & 3) * 2u + (uint32_t)(k >> 2) * (16384u >> 4);
-                    if (mma_mode == 1) umma_ss(tmem + (uint32_t)(i & 1) * 128u, da + ko, db + ko, idesc, k > 0);
-                    else umma_ts(tmem + (uint32_t)(i & 1) * 128u, tmem + 384u + 8u * k, db + ko, idesc, k > 0);
+                    // interleaved: two accumulator tiles take the K-steps in turn (kk = the K-step of the tile)
+                    const uint32_t d = tmem + (interleave ? (uint32_t)(k & 1) : (uint32_t)(i & 1)) * 128u;
+                    const uint32_t acc = interleave ? (uint32_t)(k > 1 || (i & 3) != 0) : (uint32_t)(k > 0);
+                    if (mma_mode == 1) umma_ss(d, da + ko, db + ko, idesc, acc);
+                    else umma_ts(d, tmem + 384u + 8u * k, db + ko, idesc, acc);
                 }
             }
             umma_commit(bars);
@@ -288,7 +295,7 @@ extern "C" int bfly_debug_peak(int which, int variant, int iters, double *value_
             case BFLY_PEAK_UMMA:
                 cudaFuncSetAttribute(peak_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PK_SMEM);
                 peak_umma_kernel<<<sms, PK_THREADS, PK_SMEM>>>(cyc, out, iters, variant);
-                work = (double)sms * iters * 8.0 * 2.0 * 128.0 * ((variant & 4) ? 256.0 : 128.0) * 16.0;
+                work = (double)sms * iters * 8.0 * 2.0 * 128.0 * ((variant & 64) ? 64.0 : (variant & 4) ? 256.0 : 128.0) * 16.0;
                 break;
             default:
                 set_error("unknown microbenchmark %d", which);

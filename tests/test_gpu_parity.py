@@ -165,6 +165,29 @@ def test_tensor_core_transform_against_numpy(bfly, full):
         assert np.abs(z[:n_out] - ref).max() < 3e-3
 
 
+def test_tcgen05_transform_against_numpy(bfly):
+    """bfly_debug_fft_tc5: the same transform as 64 x 128 on tcgen05.mma (DFT matrices in tensor
+    memory, fp16 operands, fp32 accumulators in TMEM): four transforms (two pairs) against numpy's
+    FFT in float64, same bars as the mma.sync transform; unit impulses reproduce the DFT columns."""
+    rng = np.random.default_rng(321)
+    y = (rng.standard_normal((4, 8192)) + 1j * rng.standard_normal((4, 8192))).astype(np.complex64)
+    z, _ = bfly.debug_fft_tc5(torch.from_numpy(y).cuda())
+    z = z.cpu().numpy()
+    ref = np.fft.ifft(y.astype(np.complex128), axis=1)[:, :4096] * 8192
+    err = np.abs(z - ref)
+    scale = np.sqrt(np.mean(np.abs(ref) ** 2))
+    assert err.max() < 4e-3 * scale and np.sqrt(np.mean(err ** 2)) < 1e-3 * scale
+    y = np.zeros((4, 8192), np.complex64)
+    ms = (1, 17 + 128 * 5, 8191, 2 * 31 + 1 + 128 * 63)
+    for r, m in enumerate(ms):
+        y[r, m] = 1.0 if r % 2 == 0 else 1.0j
+    z, _ = bfly.debug_fft_tc5(torch.from_numpy(y).cuda())
+    z = z.cpu().numpy()
+    for r, m in enumerate(ms):
+        ref = np.exp(2j * np.pi * m * np.arange(4096) / 8192) * (1.0 if r % 2 == 0 else 1.0j)
+        assert np.abs(z[r] - ref).max() < 3e-3
+
+
 # ----------------------------------------------------------------- bank parameters (A1)
 def test_bank_parameters_match_oracle_norms(bfly):
     cfg = get_config(4)
