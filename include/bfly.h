@@ -70,11 +70,15 @@ enum {
                               memory, epilogue per TMEM lane.  Executes 109x the flops of the FFT
                               forms: a cross-check and the tensor-pipe measurement, not the default.
                               Needs L >= BFLY_TC_MIN_L like BFLY_FORM_FFT_TC */
-    BFLY_FORM_FFT_TC = 3   /* the same overlap-save FFT correlate with the butterflies on the
+    BFLY_FORM_FFT_TC = 3,  /* the same overlap-save FFT correlate with the butterflies on the
                               tensor cores: small DFT matrices x data in fp16, fp32 accumulate,
                               fp32 twiddles and epilogue.  |d rho| ~ 1e-5 + 5e-5 rho.
                               Needs L >= BFLY_TC_MIN_L (BFLY_EUNSUPPORTED otherwise); the default
                               form falls back to BFLY_FORM_FFT for shorter templates */
+    BFLY_FORM_FFT_TC5 = 5  /* the same with the length-8192 transform as 64 x 128 on tcgen05.mma
+                              (DFT matrices resident in tensor memory, fp32 accumulators in TMEM,
+                              data through swizzled shared memory; csrc/bfly_fft_tc5.cu).  Needs
+                              L >= BFLY_TC_MIN_L */
 };
 #define BFLY_TC_MIN_L 256
 

@@ -17,12 +17,12 @@ from . import build as _build
 
 __all__ = ["BflyError", "Bank", "make_bank", "make_bank_grid", "correlate", "correlate_form",
            "butterfly_map", "search_host", "launch_count", "lib_path",
-           "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC",
+           "FORM_DEFAULT", "FORM_FFT", "FORM_DIRECT", "FORM_FFT_TC", "FORM_DENSE_TC", "FORM_FFT_TC5",
            "debug_fft_tc", "debug_fft_tc5", "tails", "hits_map", "time_randomize", "coincidence", "pseudo_spectrum",
            "make_bank_settle", "FAMILY_POLY", "FAMILY_SETTLE", "debug_peak", "PEAK_FFMA", "PEAK_FFMA2", "PEAK_LDS", "PEAK_HMMA", "PEAK_SHFL", "PEAK_L2",
            "PEAK_UMMA"]
 
-FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC, FORM_DENSE_TC = 0, 1, 2, 3, 4
+FORM_DEFAULT, FORM_FFT, FORM_DIRECT, FORM_FFT_TC, FORM_DENSE_TC, FORM_FFT_TC5 = 0, 1, 2, 3, 4, 5
 FAMILY_POLY, FAMILY_SETTLE = 0, 1
 PEAK_FFMA, PEAK_FFMA2, PEAK_LDS, PEAK_HMMA, PEAK_SHFL, PEAK_L2, PEAK_UMMA = range(7)
 

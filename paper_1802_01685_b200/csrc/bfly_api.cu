@@ -375,11 +375,12 @@ static int correlate_check(const bfly_bank *bank, int *form_io, const float *x_d
     // the tensor-core form needs templates long enough for its fp16 rounding errors to average
     // out; shorter ones go to the fp32 FFT form
     if (form == BFLY_FORM_DEFAULT) form = bank->L >= BFLY_TC_MIN_L ? BFLY_FORM_FFT_TC : BFLY_FORM_FFT;
-    if ((form == BFLY_FORM_FFT_TC || form == BFLY_FORM_DENSE_TC) && bank->L < BFLY_TC_MIN_L) {
+    if ((form == BFLY_FORM_FFT_TC || form == BFLY_FORM_DENSE_TC || form == BFLY_FORM_FFT_TC5) && bank->L < BFLY_TC_MIN_L) {
         set_error("the fp16-operand forms need L >= %d (L = %d)", BFLY_TC_MIN_L, bank->L);
         return BFLY_EUNSUPPORTED;
     }
-    if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT && form != BFLY_FORM_FFT_TC && form != BFLY_FORM_DENSE_TC) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
+    if (form != BFLY_FORM_FFT && form != BFLY_FORM_DIRECT && form != BFLY_FORM_FFT_TC && form != BFLY_FORM_DENSE_TC &&
+        form != BFLY_FORM_FFT_TC5) { set_error("unknown form %d", form); return BFLY_EUNSUPPORTED; }
     *form_io = form;
     return BFLY_OK;
 }
@@ -402,6 +403,8 @@ static int correlate_locked(const bfly_bank *bank, int form, const float *x_dev,
         rc = launch_dense_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
     else if (form == BFLY_FORM_FFT)
         rc = launch_fft(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
+    else if (form == BFLY_FORM_FFT_TC5)
+        rc = launch_fft_tc5(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
     else
         rc = launch_fft_tc(b, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st);
     if (rc) return rc;

@@ -24,6 +24,7 @@
 // the mma.sync transform and why.
 #include <cuda_fp16.h>
 
+#include "bfly_fft32.cuh"
 #include "bfly_internal.cuh"
 #include "bfly_tcgen05.cuh"
 
@@ -232,6 +233,531 @@ tc5_debug_kernel(const float2 *__restrict__ y, float2 *__restrict__ z, int n_pai
     if (warp == 16) tmem_dealloc(tmem, 512);
 }
 
+
+// ==========================================================================================
+// BFLY_FORM_FFT_TC5: the overlap-save FFT correlate (rows A3-A7) with the transform above.
+//
+// Per template: one "G pair" (g synthesised into a B1 tile; step 2 run with the odd-m2 half negated
+// for the second half of the pair, so that the pair's two outputs are G[0..4095] and G[4096..8191])
+// and then the blocks two at a time ("block pairs"): P (Y = X_b . G in packed fp16, B1 tile),
+// MMA step 1, T (twiddle + transpose, B2 tiles), MMA step 2, E (|z|^2 / n2, max / argmax).  The 16
+// warps run the stages of successive pairs in a fixed software-pipelined order.  There is no MMA
+// warp (17 warps would be allocated as 20 and leave 96 registers per thread): every MMA step has a
+// shared-memory counter of the arrivals it depends on, and the warp that makes the last arrival
+// issues the step and commits it to an mbarrier the consumers wait on:
+//     step 1 of pair x:  16 arrivals "B1 of x written" (P) + 16 "D1 drained" (T of pair x - 1)
+//     step 2 of pair x:  16 arrivals "B2 of x written" (T) + 16 "D2 drained" (E of pair x - 1)
+//     d1d / d2d (mbarriers, tcgen05.commit): step 1 / step 2 of the oldest outstanding pair is done
+// Tensor memory (512 columns): D1 256 | D2 128 | A_0 64 | A_1 64, all single-buffered: while the
+// warps twiddle pair p the tensor core runs step 2 of pair p - 1, then step 1 of pair p + 1.
+// Shared memory: three 64 KB tile slots (a pair's B1, overwritten in place by its B2) and G.
+constexpr int C5_THREADS = 512;
+constexpr int C5_NSLOT = 3;
+constexpr uint32_t C5_SLOT = 65536;
+constexpr uint32_t C5_OFF_G = C5_NSLOT * C5_SLOT;                 // 32 KB: G in the P-stage layout, fp16
+constexpr uint32_t C5_OFF_BAR = C5_OFF_G + 32768;                 // d1d, d2d; step counters at +32; tmem slot at +96
+constexpr uint32_t C5_OFF_RED = C5_OFF_BAR + 128;                 // [2][16] u64
+constexpr uint32_t C5_OFF_PAR = C5_OFF_RED + 256;                 // [2][32] bytes
+constexpr uint32_t C5_OFF_TAIL = C5_OFF_PAR + 64;                 // [2][16][2 MAX_TAIL] floats
+constexpr int C5_MAX_TAIL = 4;
+constexpr size_t C5_SMEM = 1024 + C5_OFF_TAIL + 2 * 16 * 2 * C5_MAX_TAIL * 4;
+constexpr float C5_GS = 0.0625f;                                   // g is synthesised times 2^-4 (fp16 headroom)
+
+// Where element m = 128 m1 + m2 of a block spectrum (and of G) lives in the P-stage layout, in
+// halves: thread t = m2 + 128 (m1 >> 4) owns 16 consecutive m1; 16-byte chunk c4 of a thread =
+// {re m1 0-7, re m1 8-15, im m1 0-7, im m1 8-15} at ((c4 512 + t) 8 + (m1 & 7)).
+__host__ __device__ __forceinline__ int c5_slot_half(int m, int comp)
+{
+    const int m1 = m >> 7, m2 = m & 127, t = m2 + 128 * (m1 >> 4), s = m1 & 15;
+    return ((2 * comp + (s >> 3)) * 512 + t) * 8 + (s & 7);
+}
+
+// Data-block spectra X_b = conj(F+(x_b 2^s)) / B in that layout (fp16) and the block scales
+// (as tc_spectra_kernel of bfly_fft_tc.cu, other scatter).
+__global__ void __launch_bounds__(fft32::NT, 1)
+c5_spectra_kernel(const float *__restrict__ x, int64_t n_samples, int64_t lag_begin,
+                  __half *__restrict__ xh, double *__restrict__ qs)
+{
+    extern __shared__ float2 c5s_smem[];
+    __shared__ float esum[fft32::NT / 32];
+    const fft32::Smem sm = fft32::carve(c5s_smem);
+    const int t = threadIdx.x;
+    fft32::fill_tables(sm, t);
+    const int64_t off = lag_begin + (int64_t)blockIdx.x * 4096;
+    float2 v[fft32::PTS];
+    float e = 0.0f;
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) {
+        const int64_t gi = off + t + fft32::NT * s;
+        const float xv = gi < n_samples ? __ldg(x + gi) : 0.0f;
+        v[s] = make_float2(xv, 0.0f);
+        e = fmaf(xv, xv, e);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((t & 31) == 0) esum[t >> 5] = e;
+    __syncthreads();
+    float tot = 0.0f;
+#pragma unroll
+    for (int w = 0; w < fft32::NT / 32; ++w) tot += esum[w];
+    float sc = 1.0f;
+    if (tot > 0.0f && isfinite(tot)) {
+        int ex;
+        frexpf(sqrtf(tot * (1.0f / (float)FFT_B)), &ex);
+        sc = ldexpf(1.0f, 1 - ex);                                // block rms in [1, 2)
+    }
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) v[s].x *= sc;
+    fft32::fft8192(v, sm, t);
+    __half *out = xh + (int64_t)blockIdx.x * 16384;
+    const float nb = 1.0f / (float)FFT_B;
+#pragma unroll
+    for (int s = 0; s < fft32::PTS; ++s) {
+        const int m = t + fft32::NT * s;
+        out[c5_slot_half(m, 0)] = __float2half_rn(v[s].x * nb);
+        out[c5_slot_half(m, 1)] = __float2half_rn(-v[s].y * nb);
+    }
+    if (t == 0) qs[blockIdx.x] = 1.0 / ((double)sc * (double)sc * (double)C5_GS * (double)C5_GS);
+}
+
+// Per-lag normaliser qs[b] / n2 in the order the E stage reads it: float index
+// b 4096 + (((q 2 + h) 32 + lane) 16 + jj) belongs to lag b 4096 + n1 + 64 n2 with
+// n2 = 16 q + (lane & 15), n1 = 32 h + 16 (lane >> 4) + jj.  -inf past the last lag.
+__global__ void __launch_bounds__(256)
+c5_norm_kernel(const float *__restrict__ x, int32_t L, int64_t lag_begin, int64_t n_fft_lags,
+               const double *__restrict__ qs, float *__restrict__ rn2p, int64_t n_slots)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_slots) return;
+    const int jj = (int)(idx & 15), lane = (int)((idx >> 4) & 31), h = (int)((idx >> 9) & 1), q = (int)((idx >> 10) & 3);
+    const int64_t b = idx >> 12;
+    const int n = (32 * h + 16 * (lane >> 4) + jj) + 64 * (16 * q + (lane & 15));
+    const int64_t i = b * 4096 + n;
+    if (i >= n_fft_lags) { rn2p[idx] = -INFINITY; return; }
+    const float *p = x + lag_begin + i;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int32_t k = 0;
+    for (; k + 4 <= L; k += 4) {
+        const double v0 = (double)__ldg(p + k), v1 = (double)__ldg(p + k + 1);
+        const double v2 = (double)__ldg(p + k + 2), v3 = (double)__ldg(p + k + 3);
+        a0 = fma(v0, v0, a0); a1 = fma(v1, v1, a1); a2 = fma(v2, v2, a2); a3 = fma(v3, v3, a3);
+    }
+    for (; k < L; ++k) { const double v = (double)__ldg(p + k); a0 = fma(v, v, a0); }
+    const double n2 = (a0 + a1) + (a2 + a3);
+    rn2p[idx] = n2 > 0.0 ? (float)(qs[b] / n2) : 0.0f;
+}
+
+__device__ __forceinline__ void named_sync_workers() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
+__device__ __forceinline__ __half2 u2h(uint32_t w) { return *reinterpret_cast<__half2 *>(&w); }
+__device__ __forceinline__ uint32_t h2u(__half2 v) { return *reinterpret_cast<uint32_t *>(&v); }
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void c5_cp_async8(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void c5_cp_async4(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
+
+// FAM as in tc_correlate_kernel: 0 linear, 1 cubic (N1), 2 settling (N2).
+template <int FAM>
+__global__ void __launch_bounds__(C5_THREADS, 1)
+c5_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA, const uint64_t *__restrict__ phB,
+                    const uint64_t *__restrict__ phC, const float *__restrict__ inc2, const float *__restrict__ ins2,
+                    const uint4 *__restrict__ xh, const float4 *__restrict__ rn2p, const float *__restrict__ x,
+                    const float *__restrict__ rn2, int64_t lag_begin, int32_t n_blocks, int32_t n_tail,
+                    float *__restrict__ rho_max, int32_t *__restrict__ arg_lag)
+{
+    extern __shared__ unsigned char c5_raw[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t base = (saddr(c5_raw) + 1023u) & ~1023u;
+    unsigned char *gbase = c5_raw + (base - saddr(c5_raw));                    // generic pointer to `base`
+    const uint32_t bars = base + C5_OFF_BAR;
+    const uint32_t D1D = bars, D2D = bars + 8, CNT1 = bars + 32, CNT2 = bars + 48, TSLOT = bars + 96;
+    if (tid == 0) {
+        bar_init(D1D, 1);
+        bar_init(D2D, 1);
+        bar_init_fence();
+        // step counters of pairs x mod 4; the first pair has no predecessor to wait for
+        for (int i = 0; i < 4; ++i) {
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(CNT1 + 4u * i), "r"(i == 0 ? 16u : 0u) : "memory");
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(CNT2 + 4u * i), "r"(i == 0 ? 16u : 0u) : "memory");
+        }
+    }
+    if (warp == 0) tmem_alloc(TSLOT, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    uint32_t tmem;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem) : "r"(TSLOT) : "memory");
+
+    const int64_t my_templates = blockIdx.x < T ? (T - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+    const int nbp = (n_blocks + 1) >> 1;                               // block pairs per template
+    const uint64_t total_pairs = (uint64_t)my_templates * (uint64_t)(nbp + 1);
+
+    {
+        // ---- the MMA steps; issued by whichever thread makes the last arrival on the step's counter
+        const uint32_t id1 = idesc_f16(128, 256), id2 = idesc_f16(128, 128);
+        auto step1 = [&](uint64_t pair) {
+            const uint32_t buf = base + (uint32_t)(pair % 3) * C5_SLOT;
+#pragma unroll
+            for (int s = 0; s < 8; ++s)
+                umma_ts(tmem + COL_D1, tmem + COL_A0 + 8u * s,
+                        smem_desc_k128(buf + (uint32_t)(s >> 2) * 32768u) + 2u * (s & 3), id1, s > 0);
+            umma_commit(D1D);
+        };
+        auto step2 = [&](uint64_t pair) {
+            const uint32_t buf = base + (uint32_t)(pair % 3) * C5_SLOT;
+#pragma unroll
+            for (int vv = 0; vv < 2; ++vv)
+#pragma unroll
+                for (int s = 0; s < 8; ++s)
+                    umma_ts(tmem + COL_D2, tmem + (vv ? COL_A1 : COL_A0) + 8u * s,
+                            smem_desc_k128(buf + (uint32_t)vv * 32768u + (uint32_t)(s >> 2) * 16384u) + 2u * (s & 3),
+                            id2, (vv | s) > 0);
+            umma_commit(D2D);
+        };
+        // one arrival (per warp, lane 0) on a step counter; true for the 32nd, which resets the counter
+        auto last_arrival = [&](uint32_t cnt_addr) -> bool {
+            uint32_t old;
+            asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(cnt_addr) : "memory");
+            if (old != 31u) return false;
+            asm volatile("st.relaxed.cta.shared::cta.u32 [%0], %1;" ::"r"(cnt_addr), "r"(0u) : "memory");
+            tc_fence_after();
+            return true;
+        };
+        const int q = warp & 3, cg = (warp >> 2) & 3, i16 = lane & 15, c = lane >> 4;
+        const int idx = 16 * q + i16;                                  // n1 (T stage) or n2 (E stage)
+        const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
+        // ---- the two DFT matrices into tensor memory
+        if (warp < 8) {
+            const int odd = cg;
+            for (int kb = 0; kb < 4; ++kb) {
+                uint32_t r[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int k = 32 * kb + 2 * j;
+                    r[j] = pack_h2f(dft_entry(idx, c, k, odd), dft_entry(idx, c, k + 1, odd));
+                }
+                tmem_st16(lane_base + (odd ? COL_A1 : COL_A0) + 16u * kb, r);
+            }
+            tmem_st_wait();
+        }
+        // ---- twiddles of this thread's 32 columns m2 = 32 cg + j (see tc5_debug_kernel)
+        float2 P2[16], S2[16];
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            const int num = ((32 * cg + j) * idx) & 8191;
+            float s, co;
+            sincospif((float)num * (1.0f / 4096.0f), &s, &co);
+            if (j & 1) { P2[j >> 1].y = co; S2[j >> 1].y = c ? -s : s; }
+            else { P2[j >> 1].x = co; S2[j >> 1].x = c ? -s : s; }
+        }
+        auto prefetch_params = [&](int64_t jn, int ps) {              // thread 0 only
+            const uint32_t d = base + C5_OFF_PAR + 32u * ps;
+            c5_cp_async8(d, phA + jn);
+            c5_cp_async8(d + 8, phB + jn);
+            if (FAM != 0) c5_cp_async8(d + 16, phC + jn);
+            c5_cp_async4(d + 24, inc2 + jn);
+            c5_cp_async4(d + 28, ins2 + jn);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        if (tid == 0 && my_templates > 0) {
+            prefetch_params(blockIdx.x, 0);
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        tc_fence_before();
+        named_sync_workers();
+        tc_fence_after();
+
+        uint64_t pc_p = 0, pc_t = 0, pc_e = 0;                         // pairs whose P / T / E stage this thread has run
+
+        // ---- P of a G pair: synthesise g of template `jt` (parameters in slot ps) into a B1 tile whose two
+        //      halves (the pair's two "blocks") both hold g; direct sums for the tail lags
+        auto stage_pg = [&](int ps) {
+            const uint32_t slot = (uint32_t)(pc_p % 3);
+            const uint32_t buf = base + slot * C5_SLOT;
+            const unsigned char *pp = gbase + C5_OFF_PAR + 32 * ps;
+            const uint64_t A = *reinterpret_cast<const uint64_t *>(pp), Bq = *reinterpret_cast<const uint64_t *>(pp + 8);
+            const uint64_t Cq = FAM != 0 ? *reinterpret_cast<const uint64_t *>(pp + 16) : 0ull;
+            const float ic = *reinterpret_cast<const float *>(pp + 24);
+            const float rq = sqrtf(*reinterpret_cast<const float *>(pp + 28) / ic);
+            int ptid = tid;
+            asm volatile("" : "+r"(ptid));                             // keep this index arithmetic out of the loop's registers
+            const int m2 = ptid & 127, mgo = (ptid >> 7) & 1, hh = ptid >> 8;
+            float tc_[C5_MAX_TAIL], ts_[C5_MAX_TAIL];
+#pragma unroll
+            for (int r = 0; r < C5_MAX_TAIL; ++r) tc_[r] = ts_[r] = 0.0f;
+            uint32_t wr[4], wi[4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                float cs[2], sn[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int n = 128 * (16 * mgo + 8 * hh + 2 * a + e) + m2;
+                    cs[e] = sn[e] = 0.0f;
+                    if (n < L) {
+                        const uint64_t p64 = FAM == 2 ? settle_phase(A, __longlong_as_double((long long)Bq),
+                                                                     __longlong_as_double((long long)Cq), (uint64_t)n)
+                                                      : template_phase(A, Bq, Cq, (uint64_t)n);
+                        const float ang = (float)(int32_t)(uint32_t)(p64 >> 32) * 1.4629180792671596e-9f;   // pi 2^-31
+                        sn[e] = __sinf(ang) * rq;
+                        cs[e] = __cosf(ang);
+                        if (n_tail > 0) {
+                            const float *xp = x + lag_begin + (int64_t)n_blocks * 4096 + n;
+#pragma unroll
+                            for (int r = 0; r < C5_MAX_TAIL; ++r) {
+                                if (r < n_tail) {
+                                    const float xv = __ldg(xp + r);
+                                    tc_[r] = fmaf(xv, cs[e], tc_[r]);
+                                    ts_[r] = fmaf(xv, sn[e], ts_[r]);
+                                }
+                            }
+                        }
+                    }
+                }
+                wr[a] = pack_h2f(cs[0] * C5_GS, cs[1] * C5_GS);
+                wi[a] = pack_h2f(-sn[0] * C5_GS, -sn[1] * C5_GS);
+            }
+            const uint32_t ch = 2u * mgo + hh;
+#pragma unroll
+            for (int blk = 0; blk < 2; ++blk) {
+                const uint32_t n = 128u * blk + m2;
+                sts128(buf + swz128(n, ch), wr[0], wr[1], wr[2], wr[3]);
+                sts128(buf + 32768u + swz128(n, ch), wi[0], wi[1], wi[2], wi[3]);
+                sts128(buf + swz128(n, 4u + ch), 0u, 0u, 0u, 0u);     // m1 >= 32: zero padding of g
+                sts128(buf + 32768u + swz128(n, 4u + ch), 0u, 0u, 0u, 0u);
+            }
+            if (n_tail > 0) {
+                float *tl = reinterpret_cast<float *>(gbase + C5_OFF_TAIL) + ps * (16 * 2 * C5_MAX_TAIL);
+#pragma unroll
+                for (int r = 0; r < C5_MAX_TAIL; ++r) {
+                    if (r >= n_tail) break;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        tc_[r] += __shfl_xor_sync(0xffffffffu, tc_[r], o);
+                        ts_[r] += __shfl_xor_sync(0xffffffffu, ts_[r], o);
+                    }
+                    if (lane == 0) { tl[(warp * C5_MAX_TAIL + r) * 2] = tc_[r]; tl[(warp * C5_MAX_TAIL + r) * 2 + 1] = ts_[r]; }
+                }
+            }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0 && last_arrival(CNT1 + 4u * (uint32_t)(pc_p & 3))) step1(pc_p);
+            ++pc_p;
+        };
+        // ---- P of a block pair: Y = X_b . G in packed fp16 straight into the B1 tile
+        auto stage_p = [&](int32_t bp) {
+            const uint32_t slot = (uint32_t)(pc_p % 3);
+            const uint32_t buf = base + slot * C5_SLOT;
+            const int m2 = tid & 127, mg = tid >> 7;
+#pragma unroll
+            for (int blk = 0; blk < 2; ++blk) {
+                const int32_t b = 2 * bp + blk;
+                const uint32_t n = 128u * blk + m2;
+                if (b < n_blocks) {
+                    const uint4 *xb = xh + (int64_t)b * 2048 + tid;
+                    const uint4 xr0 = __ldg(xb), xr1 = __ldg(xb + 512), xi0 = __ldg(xb + 1024), xi1 = __ldg(xb + 1536);
+                    const uint32_t ga = base + C5_OFF_G + 16u * tid;
+                    const uint4 gr0 = lds128(ga), gr1 = lds128(ga + 8192u), gi0 = lds128(ga + 16384u), gi1 = lds128(ga + 24576u);
+#define C5_CMUL(XR, XI, GR, GI, YR, YI)                                                       \
+    YR = h2u(__hfma2(__hneg2(u2h(XI)), u2h(GI), __hmul2(u2h(XR), u2h(GR))));                  \
+    YI = h2u(__hfma2(u2h(XI), u2h(GR), __hmul2(u2h(XR), u2h(GI))));
+                    uint4 yr0, yi0, yr1, yi1;
+                    C5_CMUL(xr0.x, xi0.x, gr0.x, gi0.x, yr0.x, yi0.x) C5_CMUL(xr0.y, xi0.y, gr0.y, gi0.y, yr0.y, yi0.y)
+                    C5_CMUL(xr0.z, xi0.z, gr0.z, gi0.z, yr0.z, yi0.z) C5_CMUL(xr0.w, xi0.w, gr0.w, gi0.w, yr0.w, yi0.w)
+                    C5_CMUL(xr1.x, xi1.x, gr1.x, gi1.x, yr1.x, yi1.x) C5_CMUL(xr1.y, xi1.y, gr1.y, gi1.y, yr1.y, yi1.y)
+                    C5_CMUL(xr1.z, xi1.z, gr1.z, gi1.z, yr1.z, yi1.z) C5_CMUL(xr1.w, xi1.w, gr1.w, gi1.w, yr1.w, yi1.w)
+#undef C5_CMUL
+                    sts128(buf + swz128(n, 2u * mg), yr0.x, yr0.y, yr0.z, yr0.w);
+                    sts128(buf + swz128(n, 2u * mg + 1u), yr1.x, yr1.y, yr1.z, yr1.w);
+                    sts128(buf + 32768u + swz128(n, 2u * mg), yi0.x, yi0.y, yi0.z, yi0.w);
+                    sts128(buf + 32768u + swz128(n, 2u * mg + 1u), yi1.x, yi1.y, yi1.z, yi1.w);
+                } else {                                               // the odd block out: zeros
+                    sts128(buf + swz128(n, 2u * mg), 0u, 0u, 0u, 0u);
+                    sts128(buf + swz128(n, 2u * mg + 1u), 0u, 0u, 0u, 0u);
+                    sts128(buf + 32768u + swz128(n, 2u * mg), 0u, 0u, 0u, 0u);
+                    sts128(buf + 32768u + swz128(n, 2u * mg + 1u), 0u, 0u, 0u, 0u);
+                }
+            }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0 && last_arrival(CNT1 + 4u * (uint32_t)(pc_p & 3))) step1(pc_p);
+            ++pc_p;
+        };
+        // ---- T: twiddle and transpose D1 -> B2 tiles (in place of the pair's B1).  G pairs negate the
+        //      odd-m2 half of their second block: its step 2 then yields G[4096 + n].
+        auto stage_t = [&](bool gpair) {
+            const uint32_t slot = (uint32_t)(pc_t % 3);
+            const uint32_t buf = base + slot * C5_SLOT;
+            bar_wait(D1D, (uint32_t)(pc_t & 1));
+            tc_fence_after();
+#pragma unroll
+            for (int blk = 0; blk < 2; ++blk) {
+                const uint32_t n = 64u * blk + idx;
+                const float sgn = (gpair && blk) ? -1.0f : 1.0f;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    uint32_t v[16];
+                    tmem_ld16(lane_base + COL_D1 + 128u * blk + 32u * cg + 16u * h, v);
+                    tmem_ld_wait();
+                    float2 o[8];
+#pragma unroll
+                    for (int a = 0; a < 8; ++a) {
+                        const float2 mine = make_float2(__uint_as_float(v[2 * a]), __uint_as_float(v[2 * a + 1]));
+                        const float2 snd = __fmul2_rn(mine, S2[8 * h + a]);
+                        float2 oth;
+                        oth.x = __shfl_xor_sync(0xffffffffu, snd.x, 16);
+                        oth.y = __shfl_xor_sync(0xffffffffu, snd.y, 16);
+                        o[a] = __ffma2_rn(mine, P2[8 * h + a], oth);
+                    }
+                    // o[a] = columns (m2 = 32 cg + 16 h + 2 a, + 1) = (u = 16 cg + 8 h + a; vv = 0, 1)
+                    const uint32_t off = (uint32_t)c * 16384u + swz128(n, 2u * cg + h);
+                    sts128(buf + off, pack_h2f(o[0].x, o[1].x), pack_h2f(o[2].x, o[3].x), pack_h2f(o[4].x, o[5].x),
+                           pack_h2f(o[6].x, o[7].x));
+                    sts128(buf + 32768u + off, pack_h2f(sgn * o[0].y, sgn * o[1].y), pack_h2f(sgn * o[2].y, sgn * o[3].y),
+                           pack_h2f(sgn * o[4].y, sgn * o[5].y), pack_h2f(sgn * o[6].y, sgn * o[7].y));
+                }
+            }
+            fence_async_smem();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+                // D1 is drained: step 1 of the next pair may run (if its B1 is there); B2 is written: step 2 of
+                // this pair may run (if D2 is drained)
+                if (pc_t + 1 < total_pairs && last_arrival(CNT1 + 4u * (uint32_t)((pc_t + 1) & 3))) step1(pc_t + 1);
+                if (last_arrival(CNT2 + 4u * (uint32_t)(pc_t & 3))) step2(pc_t);
+            }
+            ++pc_t;
+        };
+
+        int ps = 0;
+        for (int64_t it = 0, j = blockIdx.x; it < my_templates; ++it, j += gridDim.x, ps ^= 1) {
+            const float ic = *reinterpret_cast<const float *>(gbase + C5_OFF_PAR + 32 * ps + 24);
+            if (it == 0) stage_pg(0);                                  // otherwise issued two pairs ahead, below
+            if (tid == 0 && it + 1 < my_templates) prefetch_params(j + gridDim.x, ps ^ 1);
+            stage_t(true);                                             // T of this template's G pair
+            // (E of the previous template's last block pair and its output were done at the end of its iteration)
+            // ---- E of the G pair: G -> shared memory (fp16, P-stage layout)
+            {
+                bar_wait(D2D, (uint32_t)(pc_e & 1));
+                tc_fence_after();
+                uint32_t v[32];
+                tmem_ld32(lane_base + COL_D2 + 32u * cg, v);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                ++pc_e;
+                if (lane == 0 && pc_e < total_pairs && last_arrival(CNT2 + 4u * (uint32_t)(pc_e & 3))) step2(pc_e);
+                __half *gh = reinterpret_cast<__half *>(gbase + C5_OFF_G);
+                int pl = lane;
+                asm volatile("" : "+r"(pl));
+                const int n2 = 16 * q + (pl & 15), cc = pl >> 4;
+#pragma unroll
+                for (int jx = 0; jx < 32; ++jx) {
+                    const int m = 32 * (cg & 1) + jx + 64 * n2 + 4096 * (cg >> 1);
+                    gh[c5_slot_half(m, cc)] = __float2half_rn(__uint_as_float(v[jx]));
+                }
+                named_sync_workers();                                  // all of G is in place
+            }
+            float best = -1.0f;
+            int32_t code = 0;                                          // 16 b + jj
+            // ---- E of a block pair: A5-A7 on this thread's 16 lags of block 2 bp + (cg >> 1)
+            auto stage_e = [&](int32_t bp) {
+                bar_wait(D2D, (uint32_t)(pc_e & 1));
+                tc_fence_after();
+                uint32_t v[32];
+                tmem_ld32(lane_base + COL_D2 + 32u * cg, v);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                ++pc_e;
+                if (lane == 0 && pc_e < total_pairs && last_arrival(CNT2 + 4u * (uint32_t)(pc_e & 3))) step2(pc_e);
+                const int32_t b = 2 * bp + (cg >> 1);
+                if (b < n_blocks) {
+                    const float4 *rp = rn2p + ((int64_t)b * 4096 + (((q * 2 + (cg & 1)) * 32 + lane) * 16)) / 4;
+                    const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2), r3 = __ldg(rp + 3);
+                    const float rr[16] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w,
+                                          r2.x, r2.y, r2.z, r2.w, r3.x, r3.y, r3.z, r3.w};
+#pragma unroll
+                    for (int jj = 0; jj < 16; ++jj) {
+                        const float lo = __uint_as_float(v[jj]), hi = __uint_as_float(v[16 + jj]);
+                        const float slo = lo * lo, shi = hi * hi;
+                        // the real-part lanes own columns 0-15, the imaginary-part lanes 16-31
+                        const float snd = c ? slo : shi, own = c ? shi : slo;
+                        const float qv = (own + __shfl_xor_sync(0xffffffffu, snd, 16)) * rr[jj];
+                        if (qv > best) { best = qv; code = 16 * b + jj; }
+                    }
+                }
+            };
+            if (nbp > 0) stage_p(0);
+            if (nbp > 1) stage_p(1);
+            for (int32_t i = 0; i < nbp; ++i) {
+                stage_t(false);
+                if (i > 0) stage_e(i - 1);
+                if (i + 2 < nbp) stage_p(i + 2);
+                else if (i + 2 == nbp && it + 1 < my_templates) {
+                    if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
+                    named_sync_workers();                              // the next template's parameters are in place
+                    stage_pg(ps ^ 1);
+                }
+            }
+            if (nbp == 1 && it + 1 < my_templates) {                  // (nbp == 1: the branch above ran at i = -1: never)
+                if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
+                named_sync_workers();
+                stage_pg(ps ^ 1);
+            }
+            if (nbp > 0) stage_e(nbp - 1);
+            // ---- tail lags (direct sums), the CTA-wide maximum (ties to the smallest lag), output
+            if (n_tail > 0 && tid < n_tail) {
+                const float *tl = reinterpret_cast<const float *>(gbase + C5_OFF_TAIL) + ps * (16 * 2 * C5_MAX_TAIL);
+                float cs = 0.0f, sn = 0.0f;
+                for (int ww = 0; ww < 16; ++ww) { cs += tl[(ww * C5_MAX_TAIL + tid) * 2]; sn += tl[(ww * C5_MAX_TAIL + tid) * 2 + 1]; }
+                const float qv = fmaf(sn, sn, cs * cs) * __ldg(rn2 + (int64_t)n_blocks * 4096 + tid);
+                if (qv > best) { best = qv; code = 16 * n_blocks + tid; }
+            }
+            unsigned long long p = 0ull;
+            if (best > 0.0f) {
+                const int bb = code >> 4, jj = code & 15;
+                const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * 4096u + (uint32_t)(code - 16 * n_blocks)
+                                                   : (uint32_t)bb * 4096u + (uint32_t)(32 * (cg & 1) + 16 * c + jj + 64 * idx);
+                p = ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const unsigned long long o2 = __shfl_xor_sync(0xffffffffu, p, o);
+                p = o2 > p ? o2 : p;
+            }
+            unsigned long long *red = reinterpret_cast<unsigned long long *>(gbase + C5_OFF_RED) + 16 * ps;
+            if (lane == 0) red[warp] = p;
+            named_sync_workers();
+            if (tid == 0) {
+#pragma unroll
+                for (int ww = 1; ww < 16; ++ww) p = red[ww] > p ? red[ww] : p;
+                if (p == 0ull) {
+                    rho_max[j] = 0.0f;
+                    arg_lag[j] = (int32_t)lag_begin;
+                } else {
+                    rho_max[j] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ic);
+                    arg_lag[j] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, 512);
+}
 }  // namespace
 
 int launch_debug_fft_tc5(const float2 *y, float2 *z, int n_pairs, int reps, long long *cycles_dev, cudaStream_t stream)
@@ -245,6 +771,53 @@ int launch_debug_fft_tc5(const float2 *y, float2 *z, int n_pairs, int reps, long
     });
     if (rc) return rc;
     tc5_debug_kernel<<<1, T5_THREADS, T5_SMEM, stream>>>(y, z, n_pairs, reps, cycles_dev);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    return BFLY_OK;
+}
+
+}  // namespace bfly
+
+namespace bfly {
+int launch_fft_tc5(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin, int64_t lag_end,
+                   float *rho_max, int32_t *arg_lag, cudaStream_t stream)
+{
+    static PerDeviceOnce once;
+    const int rc = once.run(b->device, []() -> int {
+        BFLY_CUDA(cudaFuncSetAttribute(c5_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(c5_correlate_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C5_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(c5_correlate_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C5_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(c5_correlate_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C5_SMEM));
+        return BFLY_OK;
+    });
+    if (rc) return rc;
+    const int64_t n_lags = lag_end - lag_begin;
+    int64_t n_blocks; int32_t n_tail;
+    tc_plan(n_lags, &n_blocks, &n_tail);
+    if (n_blocks == 0)                     // a handful of lags only: the mma.sync kernel's direct sums
+        return launch_fft_tc(b, x, n_samples, lag_begin, lag_end, rho_max, arg_lag, stream);
+    if (n_lags >= (1LL << 31) - 2 * 4096) { set_error("too many lags"); return BFLY_ERANGE; }
+    if (n_blocks * 16384 > b->xh_cap || n_blocks * 4096 > b->rn2p_cap) { set_error("FFT workspace too small (internal)"); return BFLY_EINVAL; }
+    c5_spectra_kernel<<<(unsigned)n_blocks, fft32::NT, fft32::FFT_SMEM, stream>>>(x, n_samples, lag_begin, b->xh, b->qs);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    const int64_t n_slots = n_blocks * 4096;
+    c5_norm_kernel<<<(unsigned)((n_slots + 255) / 256), 256, 0, stream>>>(x, b->L, lag_begin, n_lags - n_tail, b->qs,
+                                                                          b->rn2p, n_slots);
+    count_launch();
+    BFLY_CUDA(cudaGetLastError());
+    const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
+    const int fam = b->family == BFLY_FAMILY_SETTLE ? 2 : b->has_f2 ? 1 : 0;
+    core_timer_start(b, stream);
+#define BFLY_C5_LAUNCH(FAM_)                                                                              \
+    c5_correlate_kernel<FAM_><<<(unsigned)ctas, C5_THREADS, C5_SMEM, stream>>>(                            \
+        b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh),     \
+        reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail, rho_max, arg_lag)
+    if (fam == 2) BFLY_C5_LAUNCH(2);
+    else if (fam == 1) BFLY_C5_LAUNCH(1);
+    else BFLY_C5_LAUNCH(0);
+#undef BFLY_C5_LAUNCH
+    core_timer_stop(b, stream);
     count_launch();
     BFLY_CUDA(cudaGetLastError());
     return BFLY_OK;

@@ -164,6 +164,9 @@ int64_t fft_blocks_needed(int32_t L, int64_t n_lags);
 int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                   int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int64_t tc_blocks_needed(int64_t n_lags);
+void tc_plan(int64_t n_lags, int64_t *n_blocks, int32_t *n_tail);
+int launch_fft_tc5(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
+                   int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int launch_tails_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                     int64_t lag_end, float kappa, float *sigma, int64_t capacity,
                     int32_t *hit_template, int32_t *hit_lag, float *hit_rho,

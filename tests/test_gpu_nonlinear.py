@@ -11,8 +11,8 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 
-FORMS = [pytest.param(3, id="fft_tc"), pytest.param(4, id="dense_tc"), pytest.param(1, id="fft"),
-         pytest.param(2, id="direct")]
+FORMS = [pytest.param(3, id="fft_tc"), pytest.param(5, id="fft_tc5"), pytest.param(4, id="dense_tc"),
+         pytest.param(1, id="fft"), pytest.param(2, id="direct")]
 
 
 @pytest.fixture(scope="module")

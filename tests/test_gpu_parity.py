@@ -20,8 +20,8 @@ def bfly():
     return b
 
 
-FORMS = [pytest.param(3, id="fft_tc"), pytest.param(1, id="fft"), pytest.param(2, id="direct"),
-         pytest.param(4, id="dense_tc")]
+FORMS = [pytest.param(3, id="fft_tc"), pytest.param(5, id="fft_tc5"), pytest.param(1, id="fft"),
+         pytest.param(2, id="direct"), pytest.param(4, id="dense_tc")]
 
 
 def _run(bfly, form, fs, L, f0, f1, x, lag_begin=0, lag_end=None):
@@ -77,7 +77,7 @@ def test_tiny_injection_on_a_grid_node(bfly, form):
 @pytest.mark.parametrize("fs,L,N", [(2000.0, 2000, 9000), (1000.0, 300, 1500), (4096.0, 4096, 4096),
                                      (4096.0, 4096, 12300), (512.0, 2, 40), (777.0, 1023, 9217)])
 def test_ragged_sizes(bfly, form, fs, L, N):
-    if form in (3, 4) and L < 256:
+    if form in (3, 4, 5) and L < 256:
         # the fp16-operand forms refuse templates shorter than BFLY_TC_MIN_L (too few terms for
         # the operand rounding to average out); the default form routes them to the fp32 FFT form
         with pytest.raises(bfly.BflyError):
