@@ -229,7 +229,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config, 1-based")
     ap.add_argument("--form", type=int, default=0,
-                    help="0 default (= 3), 1 fp32 FFT, 2 fp32 direct, 3 tensor-core FFT, 4 dense tcgen05")
+                    help="0 default (= 3), 1 fp32 FFT, 2 fp32 direct, 3 tensor-core FFT (mma.sync), 4 dense tcgen05, "
+                         "5 FFT with the transform on tcgen05")
     ap.add_argument("--templates", type=int, default=0,
                     help="development only: first n templates of the bank (not a bench line)")
     ap.add_argument("--cpu-seconds", type=float, default=30.0)
@@ -330,10 +331,11 @@ def main():
         # ---- roofline of the dominant kernel (the correlation core), timed live above; every
         #      denominator is measured in this run by bfly_debug_peak
         core_s = float(np.median(core_ms)) * 1e-3
-        is_fft = form in (0, 1, 3)
+        is_fft = form in (0, 1, 3, 5)
+        is_tc5 = form == 5
         is_tc = form in (0, 3) and cfg.L >= 256           # BFLY_TC_MIN_L (include/bfly.h)
         is_dense = form == 4
-        kernel = (("tc_correlate_kernel" if is_tc else "fft_correlate_kernel") if is_fft
+        kernel = (("c5_correlate_kernel" if is_tc5 else "tc_correlate_kernel" if is_tc else "fft_correlate_kernel") if is_fft
                   else "dense_tc_kernel" if is_dense else "direct_kernel")
         peaks = measure_peaks(bfly, local)
         mpath = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -385,6 +387,19 @@ def main():
                         "tightest_bound": "shared_memory" if t_smem >= t_hmma else "mma_sync",
                         "vs_tcgen05_rate": {"frac": mma_flops / core_s / 1e12 / bf16, "peak": bf16,
                                             "peak_basis": bf16_basis}}
+        elif is_tc5:
+            # executed tcgen05 flops: per pair of transforms 8 MMAs of 128 x 256 x 16 and 16 of 128 x 128 x 16;
+            # per template one G pair + ceil(n_blocks / 2) block pairs
+            n_blocks, n_tail = divmod(cfg.n_lags, 4096)
+            if n_tail > 4:
+                n_blocks += 1
+            pairs = 1 + (n_blocks + 1) // 2
+            mma_flops = T * pairs * (8 * 2 * 128 * 256 * 16 + 16 * 2 * 128 * 128 * 16)
+            roofline = {"bound": "tensor", "kernel": kernel, "achieved": mma_flops / core_s / 1e12, "peak": bf16,
+                        "unit": "TFLOP/s", "frac": mma_flops / core_s / 1e12 / bf16, "flops_per_launch": mma_flops,
+                        "flops_basis": "executed: per pair of transforms 8 tcgen05.mma 128x256x16 + 16 of 128x128x16 "
+                                       "(real-embedded 64-point DFT matrices; DESIGN.md 6.8)",
+                        "peak_basis": bf16_basis}
         elif is_dense:
             roofline = {"bound": "tensor", "kernel": kernel, "achieved": alg_flops / core_s / 1e12,
                         "peak": bf16, "unit": "TFLOP/s", "frac": alg_flops / core_s / 1e12 / bf16,
@@ -426,6 +441,18 @@ def main():
                                                "peak_basis": bf16_basis},
                                   "note": "same rows A3-A7 as a Hankel x template contraction on tcgen05; "
                                           "109x the flops of the FFT form, hence not the default"}}
+            # the FFT form with its transform on tcgen05 (BFLY_FORM_FFT_TC5), same partial bank
+            dms = []
+            for i in range(3):
+                bfly.correlate_form(dbank, 5, xd, 0, None, rho[:nd], arg[:nd])
+                if i:
+                    dms.append(dbank.core_ms())
+            t5s = float(np.mean(dms)) * 1e-3
+            other["fft_tc5"] = {"kernel": "c5_correlate_kernel", "templates": nd, "kernel_ms": t5s * 1e3,
+                                "value": correlations_per_step(cfg, nd) / t5s, "unit": UNIT,
+                                "note": "the same overlap-save FFT with the length-8192 transform as 64 x 128 on "
+                                        "tcgen05.mma (DFT matrices in tensor memory); measured slower than the "
+                                        "mma.sync transform (DESIGN.md 10), hence not the default"}
             # the paper's own reduction on the same kernel: sigma by Parseval + all tails above
             # kappa sigma (bfly_tails), whole bank, kappa = 5.5 (about 1e5 hits in noise)
             bank.set_timing(True)
@@ -452,7 +479,8 @@ def main():
             "dtype": "f16 mma operands, f32 accumulate" if (is_tc or is_dense) else "f32", "data": "synthetic",
             "config": {"workload": f"config {cfg.index} ({cfg.name})", "templates": T,
                        "n_samples": cfg.n_samples, "L": cfg.L, "lags": cfg.n_lags,
-                       "form": ("fft_tc" if is_tc else "fft") if is_fft else "dense_tc" if is_dense else "direct",
+                       "form": ("fft_tc5" if is_tc5 else "fft_tc" if is_tc else "fft") if is_fft
+                               else "dense_tc" if is_dense else "direct",
                        "l2": "inputs larger than L2 (bank parameters + outputs "
                              f"{(T * 48) >> 20} MiB per step)",
                        "parallelism": "replicas" if world > 1 else "single GPU",
