@@ -194,7 +194,7 @@ struct TcSmem {
     uint4 *xs;                 // two staging slots for X_b (filled by cp.async.bulk)
     float *xt;                 // x[first tail lag ..], L + MAX_TAIL - 1 samples at xt_slot(n) (direct tail lags)
     uint32_t *w16u;            // [2][3][32]: A fragments of W16 rows 8..15 (G transform only)
-    float *tail;               // [16 warps][2 MAX_TAIL] partial sums of the direct tail lags
+    float *tail;               // [2][16 warps][2 MAX_TAIL] partial sums of the direct tail lags
     unsigned long long *red;   // [2][16]
     unsigned char *par;        // [2][32]: {phA, phB, phC, inc2, ins2} of the template after this one
     unsigned long long *bar;   // mbarriers: [0..2] exchange buffer full, [3..4] X_b slot filled
@@ -205,7 +205,7 @@ constexpr size_t OFF_XS = OFF_GS + EXCH_WORDS * 4;
 constexpr size_t OFF_XT = OFF_XS + 2 * EXCH_WORDS * 4;
 constexpr size_t OFF_W16U = OFF_XT + (FFT_MAX_L + 32) * 4;
 constexpr size_t OFF_TAIL = OFF_W16U + 2 * 3 * 32 * 4;
-constexpr size_t OFF_RED = OFF_TAIL + 16 * 2 * MAX_TAIL * 4;
+constexpr size_t OFF_RED = OFF_TAIL + 2 * 16 * 2 * MAX_TAIL * 4;   // tail[] is double buffered by template parity
 constexpr size_t OFF_BAR = OFF_RED + 2 * 16 * 8;              // red[] is double buffered by template parity
 constexpr size_t OFF_PAR = OFF_BAR + 8 * 8;                   // two slots of prefetched bank parameters
 constexpr size_t TC_SMEM = OFF_PAR + 2 * 32;
@@ -237,6 +237,13 @@ __device__ __forceinline__ void synth_sincos(uint32_t Ahi, uint32_t Alo, uint32_
     *s = __sinf(ang);
     *c = __cosf(ang);
 }
+
+// Where thread `th`'s 16-byte operand chunk of G sits inside a 512-chunk row of sm.gs: bit 3 of the
+// thread index folded into bit 1.  The lanes of a warp that store G (transform output order) differ
+// in bits 0, 2, 3, 4, 8 of the owning thread's index, so without the fold they hit 4 of the 8
+// 16-byte bank groups (ncu: 16 wavefronts per 8-byte store instead of 4); the readers' lanes
+// differ in bits 0-4, of which the fold keeps bits 0-2 a permutation: still conflict free.
+__device__ __forceinline__ int gs_slot(int th) { return th ^ ((th >> 2) & 2); }
 
 // Index of tail-window sample n in sm.xt: a thread's lanes differ in bits 7-9 (g) and 11-12 (t)
 // of n; folding those into the bank bits makes the reads conflict free.
@@ -380,8 +387,30 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
     __syncthreads();
-    int ps = 0;                                                  // parameter slot / red[] half of this template
-    for (int64_t j = blockIdx.x; j < T; j += gridDim.x, ps ^= 1) {
+    // thread 0: combine the warps' maxima of a finished template (red[slot]) and write its outputs
+    auto write_out = [&](int64_t jo, int slot) {
+        const unsigned long long *red = sm.red + 16 * slot;
+        unsigned long long p = red[0];
+#pragma unroll
+        for (int ww = 1; ww < 16; ++ww) p = red[ww] > p ? red[ww] : p;
+        if (p == 0ull) {                                // rho = 0 at every lag (or no lag at all)
+            rho_max[jo] = 0.0f;
+            arg_lag[jo] = (int32_t)lag_begin;
+        } else {
+            const float ico = *reinterpret_cast<const float *>(sm.par + 32 * slot + 24);
+            rho_max[jo] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ico);
+            arg_lag[jo] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
+        }
+    };
+    // No CTA-wide barrier separates one template from the next: the first barrier of a template
+    // (after its synthesis) is where every warp is known to have left the previous one.  Until
+    // then a warp of template j + 1 writes only red[], tail[] (both double buffered by template
+    // parity) and the exchange buffer `wb`, whose last reader was block n_blocks - 3 of template j
+    // (finished by every warp: the writer has passed full(n_blocks - 1)).  The next template's
+    // parameters are published by the arrival of thread 0 in the front half of the last block.
+    int ps = 0;                                                  // parameter slot / red[] / tail[] half of this template
+    int64_t j = blockIdx.x;
+    for (; j < T; j += gridDim.x, ps ^= 1) {
         // ---- A3: synthesise g[n] = cos phi_n - i r sin phi_n, r = ||cos phi|| / ||sin phi||,
         //      n = 1024 a + 128 g + 16 c + d' < L, as the operand fragments of pass A (so that
         //      |z|^2 / ||cos phi||^2 is the quadrature sum); direct sums for the tail lags
@@ -392,7 +421,6 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         const uint32_t Bhi = (uint32_t)(Bq >> 32), Blo = (uint32_t)Bq;
         const float ic = *reinterpret_cast<const float *>(pp + 24);
         const float rq = sqrtf(*reinterpret_cast<const float *>(pp + 28) / ic);   // ic > 0: cos phi_0 = 1
-        if (tid == 0 && j + gridDim.x < T) prefetch_params(j + gridDim.x, ps ^ 1);
         // The index arithmetic of the per-template code below depends on the thread only, so the
         // compiler would hoist it out of the template loop and hold its results in registers all
         // through the block loop -- which is at the 128-register limit and then recomputes its OWN
@@ -472,14 +500,19 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                         ts_[r] += __shfl_xor_sync(0xffffffffu, ts_[r], o);
                     }
                     if (pl == 0) {
-                        sm.tail[(pw * MAX_TAIL + r) * 2] = tc_[r];
-                        sm.tail[(pw * MAX_TAIL + r) * 2 + 1] = ts_[r];
+                        float *tl = sm.tail + ps * (16 * 2 * MAX_TAIL);
+                        tl[(pw * MAX_TAIL + r) * 2] = tc_[r];
+                        tl[(pw * MAX_TAIL + r) * 2 + 1] = ts_[r];
                     }
                 }
             }
             chain1(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
         }
-        __syncthreads();
+        __syncthreads();                                // every warp has left the previous template
+        if (tid == 0) {
+            if (!TAILS && j != (int64_t)blockIdx.x) write_out(j - gridDim.x, ps ^ 1);
+            if (j + gridDim.x < T) prefetch_params(j + gridDim.x, ps ^ 1);     // after write_out: it reads that slot's inc2
+        }
         // ---- G = F+(g): all 16 rows of the last pass; G / S16 -> fp16 -> operand layout
         {
             uint32_t w16u[2][3];
@@ -508,9 +541,9 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 const uint32_t oR0 = __shfl_xor_sync(0xffffffffu, R0, 8), oI0 = __shfl_xor_sync(0xffffffffu, I0, 8);
                 const uint32_t oR1 = __shfl_xor_sync(0xffffffffu, R1, 8), oI1 = __shfl_xor_sync(0xffffffffu, I1, 8);
                 const int tid0 = (gb1 * 8 + (U & 7)) * 32 + (pt + 4 * (pg & 1)) * 4 + (pg >> 2);
-                const int word0 = ((U >> 4) * NT + tid0) * 4 + ((U >> 3) & 1) * 2;
+                const int word0 = ((U >> 4) * NT + gs_slot(tid0)) * 4 + ((U >> 3) & 1) * 2;
                 *reinterpret_cast<uint2 *>(gw + word0) = make_uint2(__byte_perm(R0, oR0, sel), __byte_perm(I0, oI0, sel));
-                *reinterpret_cast<uint2 *>(gw + word0 + 8) = make_uint2(__byte_perm(R1, oR1, sel), __byte_perm(I1, oI1, sel));
+                *reinterpret_cast<uint2 *>(gw + (word0 ^ 8)) = make_uint2(__byte_perm(R1, oR1, sel), __byte_perm(I1, oI1, sel));   // thread tid0 + 2
             }
         }
         __syncthreads();
@@ -519,7 +552,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             float acc = 0.0f;
 #pragma unroll
             for (int ci = 0; ci < 4; ++ci) {
-                const uint4 gq = sm.gs[ci * NT + tid];
+                const uint4 gq = sm.gs[ci * NT + gs_slot(tid)];
                 const float4 wv = __ldg(ta.wspec + ci * NT + tid);
                 const float2 r0 = __half22float2(as_h2(gq.x)), i0 = __half22float2(as_h2(gq.y));
                 const float2 r1 = __half22float2(as_h2(gq.z)), i1 = __half22float2(as_h2(gq.w));
@@ -555,7 +588,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 #pragma unroll
             for (int ci = 0; ci < 4; ++ci) {
                 const uint4 xq = xb[ci * NT];
-                const uint4 gq = sm.gs[ci * NT + tid];
+                const uint4 gq = sm.gs[ci * NT + gs_slot(tid)];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const __half2 xr = as_h2(h ? xq.z : xq.x), xi = as_h2(h ? xq.w : xq.y);
@@ -584,6 +617,11 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                           sm.bar + 3 + slot);
                 next_b = next_b + 1 == n_blocks ? 0 : next_b + 1;
                 ++issued;
+                // The next template's parameters (cp.async of thread 0, issued a whole G stage ago:
+                // this wait does not stall) become visible to every warp through thread 0's arrivals
+                // in the front halves that follow.  With n_blocks >= 2 this branch is taken in every
+                // block iteration of a template that has a successor.
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
             }
             const uint4 *rbuf = sm.exch + rb * (EXCH_WORDS / 4);
             rb = rb + 1 == N_EXCH ? 0 : rb + 1;
@@ -686,10 +724,11 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         }
         // ---- tail lags (direct sums) and the CTA-wide maximum, ties to the smallest lag
         if (n_tail > 0 && tid < n_tail) {
+            const float *tl = sm.tail + ps * (16 * 2 * MAX_TAIL);
             float c = 0.0f, s = 0.0f;
             for (int ww = 0; ww < 16; ++ww) {
-                c += sm.tail[(ww * MAX_TAIL + tid) * 2];
-                s += sm.tail[(ww * MAX_TAIL + tid) * 2 + 1];
+                c += tl[(ww * MAX_TAIL + tid) * 2];
+                s += tl[(ww * MAX_TAIL + tid) * 2 + 1];
             }
             if (TAILS) {
                 const float q = fmaf(s, s, c * c);                       // raw samples: no block scale
@@ -711,42 +750,34 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 #endif
             }
         }
-        if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");   // the next template's parameters
-        if (TAILS) {
-            __syncthreads();                            // red[], tail[], gs, exch are reused by the next template
-            continue;
+        if (n_blocks < 2) {                            // too few block iterations to publish the parameters through
+            if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();
         }
-        unsigned long long p = 0ull;
-        if (best > 0.0f) {                             // q = 0 everywhere: rho = 0 at the first lag, below
-            const int bb = code >> 3, rank = code & 7;            // rank = 4 e + i
-            const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * TCV + (uint32_t)(code - 8 * n_blocks)
-                                               : (uint32_t)bb * TCV + (uint32_t)((4 * w + (rank & 3)) +
-                                                                                 64 * (2 * t + (rank >> 2)) + 512 * g);
+        if (!TAILS) {
+            unsigned long long p = 0ull;
+            if (best > 0.0f) {                         // q = 0 everywhere: rho = 0 at the first lag (write_out)
+                const int bb = code >> 3, rank = code & 7;            // rank = 4 e + i
+                const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * TCV + (uint32_t)(code - 8 * n_blocks)
+                                                   : (uint32_t)bb * TCV + (uint32_t)((4 * w + (rank & 3)) +
+                                                                                     64 * (2 * t + (rank >> 2)) + 512 * g);
 #if BFLY_TC_EPI == 2
-            p = ((unsigned long long)(__float_as_uint(best) & 0xFFFFFFF8u) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
+                p = ((unsigned long long)(__float_as_uint(best) & 0xFFFFFFF8u) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
 #else
-            p = ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
+                p = ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
 #endif
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const unsigned long long q = __shfl_xor_sync(0xffffffffu, p, o);
-            p = q > p ? q : p;
-        }
-        unsigned long long *red = sm.red + 16 * ps;
-        if (lane == 0) red[w] = p;
-        __syncthreads();                                // also: every warp is done with gs, exch, tail[]
-        if (tid == 0) {                                 // the other threads go on to the next template
-#pragma unroll
-            for (int ww = 1; ww < 16; ++ww) p = red[ww] > p ? red[ww] : p;
-            if (p == 0ull) {                            // rho = 0 at every lag (or no lag at all)
-                rho_max[j] = 0.0f;
-                arg_lag[j] = (int32_t)lag_begin;
-            } else {
-                rho_max[j] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ic);
-                arg_lag[j] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
             }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const unsigned long long q = __shfl_xor_sync(0xffffffffu, p, o);
+                p = q > p ? q : p;
+            }
+            if (lane == 0) sm.red[16 * ps + w] = p;    // combined by thread 0 after the next template's first barrier
         }
+    }
+    if (!TAILS && blockIdx.x < T) {
+        __syncthreads();
+        if (tid == 0) write_out(j - gridDim.x, ps ^ 1);
     }
 }
 
