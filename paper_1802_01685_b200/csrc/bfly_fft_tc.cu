@@ -326,9 +326,11 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const float *__restrict__ ins2, const uint4 *__restrict__ xh,
                     const float4 *__restrict__ rn2p, const float *__restrict__ x,
                     const float *__restrict__ rn2, int64_t lag_begin, int32_t n_blocks,
-                    int32_t n_tail, float *__restrict__ rho_max, int32_t *__restrict__ arg_lag,
-                    const TailArgs ta)
+                    int32_t n_tail, int32_t n_ftail, const double *__restrict__ qs,
+                    float *__restrict__ rho_max, int32_t *__restrict__ arg_lag, const TailArgs ta)
 {
+    // n_tail: lags past the last block taken as direct sums during synthesis; n_ftail: such lags
+    // taken from the transform of the last block instead (launch_tc_common decides; one of the two is 0)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const TcSmem sm = carve_tc(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, t = lane & 3;
@@ -722,6 +724,40 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 #endif
             }
         }
+        // ---- tail lags from the transform of the last block: lag n_blocks TCV + r is its output
+        //      n = 4096 + r, i.e. row delta = 8 of the last pass (the rows chain2<FULL> adds) of unit
+        //      U = r, which belongs to warp 0 -- lane 0 holds (gamma, delta) = (0, 8).  That buffer
+        //      is intact: the next writers of it are two transforms away, behind the next barrier.
+        if (n_ftail > 0 && w == 0) {
+            const uint4 *lbuf = sm.exch + (rb == 0 ? N_EXCH - 1 : rb - 1) * (EXCH_WORDS / 4);
+            uint32_t w16u[2][3];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < 3; ++q) w16u[h][q] = sm.w16u[(h * 3 + q) * 32 + lane];
+            const float qsl = (float)__ldg(qs + (n_blocks - 1));
+#pragma unroll 1
+            for (int r = 0; r < n_ftail; ++r) {
+                cpair z, zu;
+                chain2<true, TC_HALF>(k, lbuf, r, lane, z, zu, w16u);
+                const float m2 = fmaf(zu.i.x, zu.i.x, zu.r.x * zu.r.x) * qsl;
+                if (lane == 0) {
+                    if (TAILS) {
+                        if (m2 > thr) {
+                            const unsigned long long at = atomicAdd(ta.n_hits, 1ull);
+                            if (at < (unsigned long long)ta.capacity) {
+                                ta.hit_template[at] = (int32_t)j;
+                                ta.hit_lag[at] = (int32_t)(lag_begin + (int64_t)n_blocks * TCV + r);
+                                ta.hit_rho[at] = sqrtf(m2 * rsig2);
+                            }
+                        }
+                    } else {
+                        const float q = m2 * __ldg(rn2 + (int64_t)n_blocks * TCV + r);
+                        if (q > best) { best = q; code = 8 * n_blocks + r; }
+                    }
+                }
+            }
+        }
         // ---- tail lags (direct sums) and the CTA-wide maximum, ties to the smallest lag
         if (n_tail > 0 && tid < n_tail) {
             const float *tl = sm.tail + ps * (16 * 2 * MAX_TAIL);
@@ -880,12 +916,17 @@ static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_sample
         BFLY_CUDA(cudaGetLastError());
     }
     const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
+    // The lags past the last whole block: output n = 4096 + r of the last block's transform is
+    // a valid (unwrapped) lag while 4096 + r <= B - L; then the kernel takes them from the rows
+    // delta >= 8 of that transform (n_ftail) and the synthesis carries no direct sums (n_dtail).
+    const bool tail_by_fft = n_tail > 0 && n_blocks > 0 && (int64_t)(n_tail - 1) <= (int64_t)TCV - (int64_t)b->L;
+    const int32_t n_ftail = tail_by_fft ? n_tail : 0, n_dtail = tail_by_fft ? 0 : n_tail;
     core_timer_start(b, stream);
 #define BFLY_TC_LAUNCH(TAILS_, FAM_, ARGS_)                                                            \
     tc_correlate_kernel<TAILS_, FAM_><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(                        \
         b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh), \
-        reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_tail,    \
-        rho_max, arg_lag, ARGS_)
+        reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_dtail,   \
+        n_ftail, b->qs, rho_max, arg_lag, ARGS_)
     const int fam = b->family == BFLY_FAMILY_SETTLE ? 2 : b->has_f2 ? 1 : 0;
     if (tails) {
         if (fam == 2) BFLY_TC_LAUNCH(true, 2, *tails);
