@@ -26,6 +26,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <type_traits>
 
 #include "bfly_internal.cuh"
 
@@ -174,7 +175,7 @@ __global__ void dense_prep_kernel(const float *__restrict__ x, int64_t n_samples
 // ------------------------------------------------------------------------------------------
 // The contraction.  Grid: persistent, one CTA per SM, strided over tiles of 128 templates.
 __global__ void __launch_bounds__(DT_THREADS, 1)
-dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, int family,
+dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, int family, int linear,
                 const uint64_t *__restrict__ phA, const uint64_t *__restrict__ phB,
                 const uint64_t *__restrict__ phC, const float *__restrict__ inc2, const float *__restrict__ ins2,
                 const float *__restrict__ rn2s, int64_t n_lags, int32_t n_lag_tiles,
@@ -227,6 +228,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, 
             const bool valid = j < T;
             const uint64_t A = valid ? phA[j] : 0ull, Bq = valid ? phB[j] : 0ull, Cq = valid ? phC[j] : 0ull;
             const float ic = valid ? inc2[j] : 0.0f, is = valid ? ins2[j] : 0.0f;
+            // linear chirps: w = exp(2 pi i dd), dd = 2 B the (constant) second phase difference, a tiny
+            // angle (|f1| / fs^2 cycles): two terms of the series are exact in fp32
+            const float wx = (float)(long long)(2ull * Bq) * 3.4061215800865545e-19f;   // 2 pi 2^-64
+            const float wr = fmaf(-0.5f * wx, wx, 1.0f), wi = fmaf(wx * wx * (-1.0f / 6.0f), wx, wx);
             unsigned long long best = 0ull;
             for (int32_t lt = 0; lt < n_lag_tiles; ++lt) {
                 for (int32_t kb = 0; kb < n_kb; ++kb) {
@@ -244,45 +249,96 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, 
                     // a float in [1, 2), minus 1.5 is the phase in [-1/2, 1/2) cycles: no
                     // int-to-float conversion (those share the XU pipe with sin / cos).
                     const uint64_t k0 = (uint64_t)kb * DT_K + 32u * (uint32_t)half;
-                    const uint64_t p0 = family_phase(family, A, Bq, Cq, k0), p1 = family_phase(family, A, Bq, Cq, k0 + 1),
-                                   p2 = family_phase(family, A, Bq, Cq, k0 + 2);
-                    const uint32_t d3 = family == BFLY_FAMILY_SETTLE
-                        ? (uint32_t)((family_phase(family, A, Bq, Cq, k0 + 3) - 3ull * p2 + 3ull * p1 - p0) >> 32)
-                        : (uint32_t)((6ull * Cq) >> 32);
-                    uint32_t ph = (uint32_t)(p0 >> 32) ^ 0x80000000u;
-                    uint32_t d = (uint32_t)((p1 - p0) >> 32);
-                    uint32_t dd = (uint32_t)((p2 - 2ull * p1 + p0) >> 32);
                     const bool whole = valid && (int32_t)k0 + 32 <= L;
+                    if (linear) {
+                        // Linear chirps (the default family): u_k = exp(2 pi i phi_k) by the rotation
+                        // recurrence u_{k+1} = u_k v_k, v_{k+1} = v_k w with v_k = exp(2 pi i (phi_{k+1} -
+                        // phi_k)): 8 fp32 FMAs per sample on the FMA pipe instead of two SFU calls (the XU
+                        // pipe, 16 lanes per SM, was the co-limiter of this kernel: 16384 sin/cos per
+                        // K-block = 1024 cycles, the same as the K-block's MMAs).  u and v are re-seeded
+                        // from the exact fixed-point phase at the thread's first sample of every K-block
+                        // (4 SFU calls per 32 samples); the phase error inside a run of 32 is below 2e-5 rad.
+                        const uint64_t p0 = template_phase(A, Bq, 0ull, k0), p1 = template_phase(A, Bq, 0ull, k0 + 1);
+                        const float fu = __uint_as_float(__funnelshift_r((uint32_t)(p0 >> 32) ^ 0x80000000u, 0x7Fu, 9));
+                        const float fv = __uint_as_float(__funnelshift_r((uint32_t)((p1 - p0) >> 32) ^ 0x80000000u, 0x7Fu, 9));
+                        const float au = fmaf(fu, 6.283185307179586f, -9.42477796076938f);
+                        const float av = fmaf(fv, 6.283185307179586f, -9.42477796076938f);
+                        float ur = __cosf(au), ui = __sinf(au), vr = __cosf(av), vi = __sinf(av);
+                        // the samples past L are masked only in the (rare) warps that own any: a
+                        // warp-uniform branch, so the common path carries no selects
+                        auto synth32 = [&](auto masked) {
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        uint32_t cw[4], sw[4];
+                        for (int c = 0; c < 4; ++c) {
+                            uint32_t cw[4], sw[4];
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            float cs[2], sn[2];
+                            for (int i = 0; i < 4; ++i) {
+                                float cs[2], sn[2];
 #pragma unroll
-                            for (int e = 0; e < 2; ++e) {
-                                const float f = __uint_as_float(__funnelshift_r(ph, 0x7Fu, 9));
-                                const float ang = fmaf(f, 6.283185307179586f, -9.42477796076938f);   // 2 pi (f - 1.5)
-                                cs[e] = __cosf(ang);
-                                sn[e] = __sinf(ang);
-                                if (!whole) {
-                                    const bool on = valid && (int32_t)k0 + 8 * c + 2 * i + e < L;
-                                    cs[e] = on ? cs[e] : 0.0f;
-                                    sn[e] = on ? sn[e] : 0.0f;
+                                for (int e = 0; e < 2; ++e) {
+                                    cs[e] = ur;
+                                    sn[e] = ui;
+                                    if (decltype(masked)::value) {
+                                        const bool on = valid && (int32_t)k0 + 8 * c + 2 * i + e < L;
+                                        cs[e] = on ? cs[e] : 0.0f;
+                                        sn[e] = on ? sn[e] : 0.0f;
+                                    }
+                                    const float nr = fmaf(ur, vr, -(ui * vi)), ni = fmaf(ur, vi, ui * vr);
+                                    const float mr = fmaf(vr, wr, -(vi * wi)), mi = fmaf(vr, wi, vi * wr);
+                                    ur = nr; ui = ni; vr = mr; vi = mi;
                                 }
-                                ph += d;
-                                d += dd;
-                                dd += d3;
+                                __half2 hc = __floats2half2_rn(cs[0], cs[1]), hs = __floats2half2_rn(sn[0], sn[1]);
+                                cw[i] = *reinterpret_cast<uint32_t *>(&hc);
+                                sw[i] = *reinterpret_cast<uint32_t *>(&hs);
                             }
-                            __half2 hc = __floats2half2_rn(cs[0], cs[1]), hs = __floats2half2_rn(sn[0], sn[1]);
-                            cw[i] = *reinterpret_cast<uint32_t *>(&hc);
-                            sw[i] = *reinterpret_cast<uint32_t *>(&hs);
+                            const uint32_t off = row_off + (((uint32_t)(4 * half + c) ^ row_x) << 4);
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + off), "r"(cw[0]), "r"(cw[1]),
+                                         "r"(cw[2]), "r"(cw[3]) : "memory");
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + DT_A_BYTES + off), "r"(sw[0]),
+                                         "r"(sw[1]), "r"(sw[2]), "r"(sw[3]) : "memory");
                         }
-                        const uint32_t off = row_off + (((uint32_t)(4 * half + c) ^ row_x) << 4);
-                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + off), "r"(cw[0]), "r"(cw[1]),
-                                     "r"(cw[2]), "r"(cw[3]) : "memory");
-                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + DT_A_BYTES + off), "r"(sw[0]),
-                                     "r"(sw[1]), "r"(sw[2]), "r"(sw[3]) : "memory");
+                        };
+                        if (__all_sync(0xffffffffu, whole)) synth32(std::false_type{});
+                        else synth32(std::true_type{});
+                    } else {
+                        const uint64_t p0 = family_phase(family, A, Bq, Cq, k0), p1 = family_phase(family, A, Bq, Cq, k0 + 1),
+                                       p2 = family_phase(family, A, Bq, Cq, k0 + 2);
+                        const uint32_t d3 = family == BFLY_FAMILY_SETTLE
+                            ? (uint32_t)((family_phase(family, A, Bq, Cq, k0 + 3) - 3ull * p2 + 3ull * p1 - p0) >> 32)
+                            : (uint32_t)((6ull * Cq) >> 32);
+                        uint32_t ph = (uint32_t)(p0 >> 32) ^ 0x80000000u;
+                        uint32_t d = (uint32_t)((p1 - p0) >> 32);
+                        uint32_t dd = (uint32_t)((p2 - 2ull * p1 + p0) >> 32);
+    #pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            uint32_t cw[4], sw[4];
+    #pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                float cs[2], sn[2];
+    #pragma unroll
+                                for (int e = 0; e < 2; ++e) {
+                                    const float f = __uint_as_float(__funnelshift_r(ph, 0x7Fu, 9));
+                                    const float ang = fmaf(f, 6.283185307179586f, -9.42477796076938f);   // 2 pi (f - 1.5)
+                                    cs[e] = __cosf(ang);
+                                    sn[e] = __sinf(ang);
+                                    if (!whole) {
+                                        const bool on = valid && (int32_t)k0 + 8 * c + 2 * i + e < L;
+                                        cs[e] = on ? cs[e] : 0.0f;
+                                        sn[e] = on ? sn[e] : 0.0f;
+                                    }
+                                    ph += d;
+                                    d += dd;
+                                    dd += d3;
+                                }
+                                __half2 hc = __floats2half2_rn(cs[0], cs[1]), hs = __floats2half2_rn(sn[0], sn[1]);
+                                cw[i] = *reinterpret_cast<uint32_t *>(&hc);
+                                sw[i] = *reinterpret_cast<uint32_t *>(&hs);
+                            }
+                            const uint32_t off = row_off + (((uint32_t)(4 * half + c) ^ row_x) << 4);
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + off), "r"(cw[0]), "r"(cw[1]),
+                                         "r"(cw[2]), "r"(cw[3]) : "memory");
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + DT_A_BYTES + off), "r"(sw[0]),
+                                         "r"(sw[1]), "r"(sw[2]), "r"(sw[3]) : "memory");
+                        }
                     }
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor-core reads
                     bar_arrive(full(stage));
@@ -444,7 +500,7 @@ int launch_dense_tc(bfly_bank *b, const float *x, int64_t n_samples, int64_t lag
     const int64_t ctas = std::min<int64_t>(n_ttiles, b->sm_count);
     core_timer_start(b, stream);
     dense_tc_kernel<<<(unsigned)ctas, DT_THREADS, DT_SMEM, stream>>>(
-        map, b->T, b->L, b->family, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->rn2s, n_lags, (int32_t)n_lag_tiles, lag_begin,
+        map, b->T, b->L, b->family, (b->family == BFLY_FAMILY_POLY && !b->has_f2) ? 1 : 0, b->phA, b->phB, b->phC, b->inc2, b->ins2, b->rn2s, n_lags, (int32_t)n_lag_tiles, lag_begin,
         rho_max, arg_lag);
     core_timer_stop(b, stream);
     count_launch();
