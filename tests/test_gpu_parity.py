@@ -106,6 +106,34 @@ def test_lag_subrange_and_empty_range(bfly, form):
     assert np.all(rho.cpu().numpy() == 0.0) and np.all(arg.cpu().numpy() == 123)
 
 
+@pytest.mark.parametrize("form", [pytest.param(3, id="fft_tc"), pytest.param(5, id="fft_tc5")])
+@pytest.mark.parametrize("fs,L,n_whole", [(2048.0, 2048, 1), (4096.0, 4096, 2), (4094.0, 4094, 1), (1000.0, 300, 3)])
+def test_lags_past_the_last_whole_block(bfly, form, fs, L, n_whole):
+    """n_lags = n_whole x 4096 + r, r = 1 .. 4: the FFT forms take the last r lags either from the
+    rows delta >= 8 of the last block's transform (while 4096 + r - 1 <= 8192 - L: all r at L = 2048
+    and 300, r <= 3 at L = 4094, r = 1 at L = 4096) or as direct sums in the synthesis; a chirp
+    injected at the very end of the range puts the maximum of its template on those lags."""
+    rng = np.random.default_rng(int(L) + n_whole)
+    T = 21
+    f0 = rng.uniform(0.05 * fs, 0.4 * fs, T)
+    f1 = rng.uniform(-0.1 * fs, 0.1 * fs, T)
+    for r in (1, 2, 3, 4):
+        n_lags = n_whole * 4096 + r
+        lb = 37
+        N = lb + n_lags + L - 1 + 11
+        x = rng.standard_normal(N)
+        last = lb + n_lags - 1
+        hc, _ = oracle.template(fs, L, f0[3], f1[3])
+        x[last:last + L] += 0.5 * hc                      # template 3 peaks on the last lag of the range
+        x = x.astype(np.float32)
+        _, rho, arg = _run(bfly, form, fs, L, f0, f1, x, lb, lb + n_lags)
+        rho_n, arg_n = rho.cpu().numpy(), arg.cpu().numpy()
+        check_values_and_argmax(x, fs, L, f0, f1, rho_n, arg_n, lb, lb + n_lags)
+        assert rho_n[3] > 0.25
+        if L >= 2048:                                     # (a 300-sample template's peak is broad)
+            assert last - int(arg_n[3]) <= 3
+
+
 @pytest.mark.parametrize("form", FORMS)
 def test_degenerate_inputs(bfly, form):
     fs, L, N = 1024.0, 512, 3000

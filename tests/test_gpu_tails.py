@@ -123,7 +123,7 @@ def test_tails_lag_subrange_scale_and_edges(bfly):
     fs, L, N = 1024.0, 512, 20000
     x = rng.standard_normal(N).astype(np.float32)
     f0, f1 = rng.uniform(50, 450, 9), rng.uniform(-150, 150, 9)
-    for lb, le in ((0, N - L + 1), (1234, 9000), (17, 17 + 4096), (17, 17 + 4097), (500, 501)):
+    for lb, le in ((0, N - L + 1), (1234, 9000), (17, 17 + 4096), (17, 17 + 4097), (17, 17 + 8192 + 4), (500, 501)):
         _, sig, hj, hl, hr, total, _ = _tails(bfly, fs, L, f0, f1, x, 3.5, 1 << 16, lb, le)
         check_tails(x, fs, L, f0, f1, 3.5, sig, hj, hl, hr, total, lb, le)
     xs = (x * np.float32(4096.0)).astype(np.float32)          # rho_sigma is scale invariant
@@ -136,6 +136,24 @@ def test_tails_lag_subrange_scale_and_edges(bfly):
         _tails(bfly, 512.0, 64, [50.0], [1.0], x, 3.5, 16)
     with pytest.raises(bfly.BflyError):                       # kappa must be > 0
         _tails(bfly, fs, L, f0, f1, x, 0.0, 16)
+
+
+@pytest.mark.parametrize("fs,L", [(1024.0, 512), (4096.0, 4096)])
+def test_tails_hits_on_the_lags_past_the_last_whole_block(bfly, fs, L):
+    """n_lags = 4096 + r: the last r lags come from the rows delta >= 8 of the last block's transform
+    (L = 512: all r; L = 4096: r = 1) or from direct sums; a chirp injected there makes them hits."""
+    rng = np.random.default_rng(int(L))
+    f0, f1 = rng.uniform(0.05 * fs, 0.4 * fs, 7), rng.uniform(-0.1 * fs, 0.1 * fs, 7)
+    for r in (1, 2, 4):
+        lb, n_lags = 23, 4096 + r
+        N = lb + n_lags + L - 1 + 5
+        x = rng.standard_normal(N)
+        hc, _ = oracle.template(fs, L, f0[2], f1[2])
+        x[lb + n_lags - 1:lb + n_lags - 1 + L] += 0.6 * hc
+        x = x.astype(np.float32)
+        _, sig, hj, hl, hr, total, _ = _tails(bfly, fs, L, f0, f1, x, 4.0, 1 << 16, lb, lb + n_lags)
+        check_tails(x, fs, L, f0, f1, 4.0, sig, hj, hl, hr, total, lb, lb + n_lags)
+        assert np.any((hj == 2) & (hl == lb + n_lags - 1))
 
 
 def test_tails_full_bank_config4_sampled_against_the_oracle(bfly):
