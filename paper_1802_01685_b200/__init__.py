@@ -60,6 +60,7 @@ def _load():
     lib.bfly_bank_reserve.argtypes = [vp, i64]
     lib.bfly_correlate.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
     lib.bfly_correlate_form.argtypes = [vp, C.c_int, vp, i64, i64, i64, vp, vp, vp]
+    lib.bfly_correlate_multi.argtypes = [vp, i32, vp, i64, i64, i64, vp, vp, vp]
     lib.bfly_butterfly_map.argtypes = [vp, vp, vp, f32, i64, i32, f64, f64, i32, i32, vp, vp, vp]
     lib.bfly_tails.argtypes = [vp, vp, i64, i64, i64, f32, vp, i64, vp, vp, vp, vp, vp]
     lib.bfly_hits_map.argtypes = [vp, vp, vp, i64, i64, i32, f64, f64, i32, i32, vp, vp, vp]
@@ -76,7 +77,7 @@ def _load():
     lib.bfly_launch_count.argtypes = []
     lib.bfly_launch_count.restype = i64
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
-                 "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_butterfly_map",
+                 "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_correlate_multi", "bfly_butterfly_map",
                  "bfly_search_host", "bfly_debug_fft_tc", "bfly_debug_fft_tc5", "bfly_tails", "bfly_hits_map",
                  "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum",
                  "bfly_make_bank3", "bfly_bank_get_f2", "bfly_debug_peak", "bfly_make_bank_settle",
@@ -243,6 +244,28 @@ def correlate_form(bank: Bank, form: int, x: torch.Tensor, lag_begin: int = 0,
 def correlate(bank: Bank, x: torch.Tensor, lag_begin: int = 0, lag_end: int | None = None,
               rho_max: torch.Tensor | None = None, arg_lag: torch.Tensor | None = None):
     return correlate_form(bank, FORM_DEFAULT, x, lag_begin, lag_end, rho_max, arg_lag)
+
+
+def correlate_multi(bank: Bank, xs, lag_begin: int = 0, lag_end: int | None = None):
+    """bfly_correlate_multi: several segments of equal length (a sequence of CUDA tensors) against
+    the same bank in one call; returns (list of rho_max, list of arg_lag), one pair per segment."""
+    xs = list(xs)
+    if not xs:
+        raise ValueError("no segments")
+    T, n, S = len(bank), xs[0].numel(), len(xs)
+    if any(x.numel() != n for x in xs):
+        raise ValueError("the segments must have equal length")
+    lag_end = n - bank.L + 1 if lag_end is None else lag_end
+    dev = torch.device("cuda", bank.device)
+    rho = [torch.empty(T, dtype=torch.float32, device=dev) for _ in range(S)]
+    arg = [torch.empty(T, dtype=torch.int32, device=dev) for _ in range(S)]
+    PA = C.c_void_p * S
+    xp = PA(*[_dev(x, torch.float32, "x", bank.device).value for x in xs])
+    rp = PA(*[t.data_ptr() for t in rho])
+    ap = PA(*[t.data_ptr() for t in arg])
+    _check(_lib.bfly_correlate_multi(bank._h, S, xp, n, int(lag_begin), int(lag_end), rp, ap,
+                                     _stream(bank.device)), "bfly_correlate_multi")
+    return rho, arg
 
 
 def butterfly_map(bank: Bank, rho_max: torch.Tensor, arg_lag: torch.Tensor, kappa: float,

@@ -106,6 +106,18 @@ static int reserve_for(bfly_bank *b, int64_t n_samples)
     return grow(&b->qs, &b->qs_cap, nb);
 }
 
+// the same for n_seg equal-length segments in one launch (launch_fft_tc_multi)
+static int reserve_for_multi(bfly_bank *b, int64_t n_samples, int n_seg)
+{
+    int rc = reserve_for(b, n_samples);
+    if (rc || n_samples < b->L) return rc;
+    const int64_t n_lags = n_samples - b->L + 1, nb = tc_blocks_needed(n_lags);
+    if ((rc = grow(&b->rn2, &b->rn2_cap, n_seg * n_lags))) return rc;
+    if ((rc = grow(&b->xh, &b->xh_cap, n_seg * nb * 2 * FFT_B))) return rc;
+    if ((rc = grow(&b->rn2p, &b->rn2p_cap, n_seg * nb * (FFT_B / 2)))) return rc;
+    return grow(&b->qs, &b->qs_cap, n_seg * nb);
+}
+
 }  // namespace bfly
 
 using namespace bfly;
@@ -139,6 +151,7 @@ void bfly_free_bank(bfly_bank *b)
     cudaFree(b->ys); cudaFree(b->rn2s); cudaFree(b->maxbits); cudaFree(b->racf); cudaFree(b->wspec);
     cudaFree(b->s_finf); cudaFree(b->s_delta); cudaFree(b->s_tc);
     cudaFree(b->packed); cudaFree(b->x_stage); cudaFree(b->rho_stage); cudaFree(b->arg_stage);
+    cudaFree(b->rho_multi); cudaFree(b->arg_multi);
     cudaFree(b->map_stage); cudaFree(b->cnt_stage);
     if (b->ws_event) cudaEventDestroy(b->ws_event);
     if (b->ev_start) cudaEventDestroy(b->ev_start);
@@ -411,6 +424,56 @@ static int correlate_locked(const bfly_bank *bank, int form, const float *x_dev,
     return ws_end(b, st);
 }
 
+// n_seg <= 4 segments of equal length, the same lag range in each, arguments checked, bank locked:
+// one launch of the default form when every lag comes from a transform, else one call per segment
+static int correlate_multi_locked(const bfly_bank *bank, int n_seg, const float *const *x_dev, int64_t n_samples,
+                                  int64_t lag_begin, int64_t lag_end, float *const *rho_max_dev,
+                                  int32_t *const *arg_lag_dev, void *stream)
+{
+    bfly_bank *b = const_cast<bfly_bank *>(bank);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n_lags = lag_end - lag_begin;
+    if (n_seg < 2 || !tc_multi_supported(b->L, n_lags)) {
+        const int form = b->L >= BFLY_TC_MIN_L ? BFLY_FORM_FFT_TC : BFLY_FORM_FFT;
+        for (int sg = 0; sg < n_seg; ++sg) {
+            const int rc = correlate_locked(bank, form, x_dev[sg], n_samples, lag_begin, lag_end, rho_max_dev[sg],
+                                            arg_lag_dev[sg], stream);
+            if (rc) return rc;
+        }
+        return BFLY_OK;
+    }
+    int rc = ws_begin(b, st);
+    if (rc) return rc;
+    if ((rc = reserve_for_multi(b, n_samples, n_seg))) return rc;
+    for (int sg = 0; sg < n_seg; ++sg)
+        if ((rc = launch_sliding_norm(x_dev[sg], n_samples, b->L, lag_begin, n_lags, b->rn2 + (int64_t)sg * n_lags, st)))
+            return rc;
+    if ((rc = launch_fft_tc_multi(b, n_seg, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev, st))) return rc;
+    return ws_end(b, st);
+}
+
+int bfly_correlate_multi(const bfly_bank *bank, int32_t n_segments, const float *const *x_dev, int64_t n_samples,
+                         int64_t lag_begin, int64_t lag_end, float *const *rho_max_dev,
+                         int32_t *const *arg_lag_dev, void *stream)
+{
+    if (!bank || !x_dev || !rho_max_dev || !arg_lag_dev) { set_error("null pointer"); return BFLY_EINVAL; }
+    if (n_segments < 1) { set_error("n_segments must be >= 1"); return BFLY_EINVAL; }
+    for (int32_t sg = 0; sg < n_segments; ++sg) {
+        int form = BFLY_FORM_DEFAULT;
+        const int rc = correlate_check(bank, &form, x_dev[sg], n_samples, lag_begin, lag_end, rho_max_dev[sg], arg_lag_dev[sg]);
+        if (rc) return rc;
+    }
+    BFLY_ENTER(bank);
+    BFLY_LOCK(bank);
+    for (int32_t s0 = 0; s0 < n_segments; s0 += 4) {
+        const int g = n_segments - s0 < 4 ? n_segments - s0 : 4;
+        const int rc = correlate_multi_locked(bank, g, x_dev + s0, n_samples, lag_begin, lag_end, rho_max_dev + s0,
+                                              arg_lag_dev + s0, stream);
+        if (rc) return rc;
+    }
+    return BFLY_OK;
+}
+
 int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int64_t n_samples,
                         int64_t lag_begin, int64_t lag_end, float *rho_max_dev,
                         int32_t *arg_lag_dev, void *stream)
@@ -591,26 +654,61 @@ int bfly_search_host(bfly_bank *b, const float *x_host, int64_t n_samples, int64
     const int64_t total_lags = n_samples - b->L + 1;
     // a single chunk takes every valid lag; otherwise hop = chunk - L (reading C11)
     const int64_t hop = (chunk_samples >= n_samples) ? total_lags : chunk_samples - b->L;
-    for (int64_t start = 0; start < total_lags; start += hop) {
-        const int64_t n = (chunk_samples < n_samples - start) ? chunk_samples : n_samples - start;
-        const int64_t lags_here = n - b->L + 1;
-        const bool last = start + hop >= total_lags;
-        const int64_t lag_end = last ? lags_here : (hop < lags_here ? hop : lags_here);
-        BFLY_CUDA(cudaMemcpyAsync(b->x_stage, x_host + start, sizeof(float) * (size_t)n,
-                                  cudaMemcpyHostToDevice, st));
+    // Consecutive chunks of equal length and equal lag range go through one launch, up to four at
+    // a time (bfly_correlate_multi: synthesis and the transform of g once per template for all of
+    // them); results and map are those of chunk-by-chunk calls, bit for bit.
+    const int64_t n_chunks = (total_lags + hop - 1) / hop;
+    const int max_group = n_chunks >= 3 ? (n_chunks - 1 < 4 ? (int)(n_chunks - 1) : 4) : 1;   // (the last chunk is ragged)
+    if (max_group > 1) {
+        if ((rc = grow(&b->x_stage, &b->x_stage_cap, (int64_t)max_group * chunk_samples))) return rc;
+        if ((rc = grow(&b->rho_multi, &b->rho_multi_cap, (int64_t)max_group * b->T))) return rc;
+        if ((rc = grow(&b->arg_multi, &b->arg_multi_cap, (int64_t)max_group * b->T))) return rc;
+        if ((rc = reserve_for_multi(b, chunk_samples, max_group))) return rc;
+    }
+    const float *last_rho = b->rho_stage;
+    const int32_t *last_arg = b->arg_stage;
+    int64_t start = 0;
+    bool done = false;
+    while (!done && start < total_lags) {
+        int64_t starts[4], n0 = 0, lag_end0 = 0;
+        int g = 0;
+        for (; g < max_group && !done && start < total_lags; ++g) {
+            const int64_t n = (chunk_samples < n_samples - start) ? chunk_samples : n_samples - start;
+            const int64_t lags_here = n - b->L + 1;
+            const bool last = start + hop >= total_lags;
+            const int64_t lag_end = last ? lags_here : (hop < lags_here ? hop : lags_here);
+            if (g == 0) { n0 = n; lag_end0 = lag_end; }
+            else if (n != n0 || lag_end != lag_end0) break;      // another shape: next group
+            starts[g] = start;
+            if (last) done = true;
+            start += hop;
+        }
+        float *rho_p[4];
+        int32_t *arg_p[4];
+        const float *x_p[4];
+        for (int i = 0; i < g; ++i) {
+            float *xs = b->x_stage + (int64_t)i * chunk_samples;
+            BFLY_CUDA(cudaMemcpyAsync(xs, x_host + starts[i], sizeof(float) * (size_t)n0, cudaMemcpyHostToDevice, st));
+            x_p[i] = xs;
+            rho_p[i] = g > 1 ? b->rho_multi + (int64_t)i * b->T : b->rho_stage;
+            arg_p[i] = g > 1 ? b->arg_multi + (int64_t)i * b->T : b->arg_stage;
+        }
         int form = BFLY_FORM_DEFAULT;
-        rc = correlate_check(b, &form, b->x_stage, n, 0, lag_end, b->rho_stage, b->arg_stage);
+        rc = correlate_check(b, &form, x_p[0], n0, 0, lag_end0, rho_p[0], arg_p[0]);
         if (rc) return rc;
-        rc = correlate_locked(b, form, b->x_stage, n, 0, lag_end, b->rho_stage, b->arg_stage, st);
+        rc = correlate_multi_locked(b, g, x_p, n0, 0, lag_end0, rho_p, arg_p, st);
         if (rc) return rc;
-        rc = launch_map(b, b->rho_stage, b->arg_stage, kappa, start, samples_per_tbin, f_lo_hz, df_hz,
-                        n_fbins, n_tbins, b->map_stage, b->cnt_stage, st);
-        if (rc) return rc;
-        if (last) break;
+        for (int i = 0; i < g; ++i) {
+            rc = launch_map(b, rho_p[i], arg_p[i], kappa, starts[i], samples_per_tbin, f_lo_hz, df_hz,
+                            n_fbins, n_tbins, b->map_stage, b->cnt_stage, st);
+            if (rc) return rc;
+        }
+        last_rho = rho_p[g - 1];
+        last_arg = arg_p[g - 1];
     }
     const size_t T = (size_t)b->T;
-    if (rho_max_host) BFLY_CUDA(cudaMemcpyAsync(rho_max_host, b->rho_stage, T * sizeof(float), cudaMemcpyDeviceToHost, st));
-    if (arg_lag_host) BFLY_CUDA(cudaMemcpyAsync(arg_lag_host, b->arg_stage, T * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    if (rho_max_host) BFLY_CUDA(cudaMemcpyAsync(rho_max_host, last_rho, T * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (arg_lag_host) BFLY_CUDA(cudaMemcpyAsync(arg_lag_host, last_arg, T * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     if (map_host) BFLY_CUDA(cudaMemcpyAsync(map_host, b->map_stage, sizeof(uint32_t) * (size_t)cells, cudaMemcpyDeviceToHost, st));
     if (counters_host) BFLY_CUDA(cudaMemcpyAsync(counters_host, b->cnt_stage, 2 * sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
     BFLY_CUDA(cudaStreamSynchronize(st));

@@ -33,19 +33,6 @@ using namespace tc;
 #endif
 constexpr bool TC_HALF = BFLY_TC_HALF != 0;
 
-// In-thread argmax of the block loop: 1 = compares in lag order (four values held back per
-// block), 2 = rank carried in the low mantissa bits + FMNMX3 tree, 0 = round-1 order (an exact
-// tie between lags l + 64 and l + 1 went to the larger lag).  Measured at config 4: see DESIGN.md.
-#ifndef BFLY_TC_EPI
-#define BFLY_TC_EPI 1
-#endif
-// Half of the warps of every scheduler run the two halves of a block iteration in the other order.
-#ifndef BFLY_TC_PEEL
-#define BFLY_TC_PEEL 0
-#endif
-#ifndef BFLY_TC_DEPHASE
-#define BFLY_TC_DEPHASE 0
-#endif
 typedef ConstsT<TC_HALF> Consts;
 
 // ------------------------------------------------------------------------------------------
@@ -206,7 +193,7 @@ constexpr size_t OFF_XT = OFF_XS + 2 * EXCH_WORDS * 4;
 constexpr size_t OFF_W16U = OFF_XT + (FFT_MAX_L + 32) * 4;
 constexpr size_t OFF_TAIL = OFF_W16U + 2 * 3 * 32 * 4;
 constexpr size_t OFF_RED = OFF_TAIL + 2 * 16 * 2 * MAX_TAIL * 4;   // tail[] is double buffered by template parity
-constexpr size_t OFF_BAR = OFF_RED + 2 * 16 * 8;              // red[] is double buffered by template parity
+constexpr size_t OFF_BAR = OFF_RED + 2 * 4 * 16 * 8;          // red[parity][segment][warp]
 constexpr size_t OFF_PAR = OFF_BAR + 8 * 8;                   // two slots of prefetched bank parameters
 constexpr size_t TC_SMEM = OFF_PAR + 2 * 32;
 __device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
@@ -316,19 +303,37 @@ struct TailArgs {
     unsigned long long *n_hits;
 };
 
+// Several data segments of equal length against the same bank in one launch (bfly_correlate_multi:
+// the two detectors of PAPER.md:124, or consecutive chunks of a stream): the blocks of segment s
+// are blocks s n_blocks .. (s + 1) n_blocks - 1 of xh / rn2p / qs; synthesis and the transform of g
+// are done once per template, max / argmax per (template, segment).
+constexpr int MAX_SEG = 4;
+struct SegArgs {
+    int32_t n_seg;
+    const float *rn2[MAX_SEG];     // 1 / n2 of the segment's lags (tail lags)
+    int64_t lag_begin[MAX_SEG];    // added to the block-relative lag of the maximum
+    float *rho_max[MAX_SEG];
+    int32_t *arg_lag[MAX_SEG];
+};
+
 // FAM: 0 = linear chirps (32-bit phase arithmetic), 1 = cubic phase (reading N1, 64-bit Horner),
 // 2 = exponentially settling chirps (reading N2: phB / phC carry the doubles D tc and 1/(fs tc)).
-template <bool TAILS, int FAM>
+// MULTI: several segments per launch (SegArgs; max / argmax mode only).  A separate instantiation,
+// so that the single-segment kernel -- the headline path -- is compiled exactly as without it.
+template <bool TAILS, int FAM, bool MULTI>
 __global__ void __launch_bounds__(NT, 1)
 tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     const uint64_t *__restrict__ phB, const uint64_t *__restrict__ phC,
                     const float *__restrict__ inc2,
                     const float *__restrict__ ins2, const uint4 *__restrict__ xh,
                     const float4 *__restrict__ rn2p, const float *__restrict__ x,
-                    const float *__restrict__ rn2, int64_t lag_begin, int32_t n_blocks,
-                    int32_t n_tail, int32_t n_ftail, const double *__restrict__ qs,
-                    float *__restrict__ rho_max, int32_t *__restrict__ arg_lag, const TailArgs ta)
+                    const float *__restrict__ rn2, int64_t lag_begin,
+                    int32_t n_blocks, int32_t n_tail, int32_t n_ftail, const double *__restrict__ qs,
+                    float *__restrict__ rho_max, int32_t *__restrict__ arg_lag, const SegArgs sa, const TailArgs ta)
 {
+    // single segment: rn2, lag_begin, rho_max, arg_lag; MULTI: the same per segment in sa (the direct
+    // tail sums and the tails mode are single-segment)
+    const int32_t n_seg = MULTI ? sa.n_seg : 1;
     // n_tail: lags past the last block taken as direct sums during synthesis; n_ftail: such lags
     // taken from the transform of the last block instead (launch_tc_common decides; one of the two is 0)
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -361,7 +366,8 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
     const uint32_t nowu[2][3] = {{0, 0, 0}, {0, 0, 0}};
     // templates of this CTA and the running sequence of its blocks (thread 0 issues the copies)
     const int64_t my_templates = blockIdx.x < T ? (T - 1 - blockIdx.x) / gridDim.x + 1 : 0;
-    const uint64_t total_blocks = (uint64_t)my_templates * (uint64_t)n_blocks;
+    const int32_t seq_blocks = MULTI ? n_blocks * n_seg : n_blocks;   // blocks per template, all segments
+    const uint64_t total_blocks = (uint64_t)my_templates * (uint64_t)seq_blocks;
     uint64_t issued = 0;                               // thread 0: X_b copies issued so far
     int32_t next_b = 0;                                // thread 0: block index of copy `issued`
     if (tid == 0)
@@ -369,7 +375,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             mbar_expect_tx(sm.bar + 3 + (int)issued, XB_BYTES);
             bulk_load(sm.xs + issued * (EXCH_WORDS / 4), xh + (int64_t)next_b * (EXCH_WORDS / 4), XB_BYTES,
                       sm.bar + 3 + (int)issued);
-            next_b = next_b + 1 == n_blocks ? 0 : next_b + 1;
+            next_b = next_b + 1 == seq_blocks ? 0 : next_b + 1;
         }
     uint32_t xcnt = 0;                                 // blocks consumed: slot = xcnt & 1, parity = (xcnt >> 1) & 1
     int wb = 0, rb = 0;                                // exchange buffer written next / read next
@@ -391,17 +397,34 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
     __syncthreads();
     // thread 0: combine the warps' maxima of a finished template (red[slot]) and write its outputs
     auto write_out = [&](int64_t jo, int slot) {
-        const unsigned long long *red = sm.red + 16 * slot;
-        unsigned long long p = red[0];
+        if (!MULTI) {
+            const unsigned long long *red = sm.red + 16 * slot;
+            unsigned long long p = red[0];
 #pragma unroll
-        for (int ww = 1; ww < 16; ++ww) p = red[ww] > p ? red[ww] : p;
-        if (p == 0ull) {                                // rho = 0 at every lag (or no lag at all)
-            rho_max[jo] = 0.0f;
-            arg_lag[jo] = (int32_t)lag_begin;
-        } else {
-            const float ico = *reinterpret_cast<const float *>(sm.par + 32 * slot + 24);
-            rho_max[jo] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ico);
-            arg_lag[jo] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
+            for (int ww = 1; ww < 16; ++ww) p = red[ww] > p ? red[ww] : p;
+            if (p == 0ull) {                            // rho = 0 at every lag (or no lag at all)
+                rho_max[jo] = 0.0f;
+                arg_lag[jo] = (int32_t)lag_begin;
+            } else {
+                const float ico = *reinterpret_cast<const float *>(sm.par + 32 * slot + 24);
+                rho_max[jo] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ico);
+                arg_lag[jo] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
+            }
+            return;
+        }
+        const float ico = *reinterpret_cast<const float *>(sm.par + 32 * slot + 24);
+        for (int sg = 0; sg < n_seg; ++sg) {
+            const unsigned long long *red = sm.red + 16 * (MAX_SEG * slot + sg);
+            unsigned long long p = red[0];
+#pragma unroll
+            for (int ww = 1; ww < 16; ++ww) p = red[ww] > p ? red[ww] : p;
+            if (p == 0ull) {                            // rho = 0 at every lag (or no lag at all)
+                sa.rho_max[sg][jo] = 0.0f;
+                sa.arg_lag[sg][jo] = (int32_t)sa.lag_begin[sg];
+            } else {
+                sa.rho_max[sg][jo] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ico);
+                sa.arg_lag[sg][jo] = (int32_t)(sa.lag_begin[sg] + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
+            }
         }
     };
     // No CTA-wide barrier separates one template from the next: the first barrier of a template
@@ -548,8 +571,14 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 *reinterpret_cast<uint2 *>(gw + (word0 ^ 8)) = make_uint2(__byte_perm(R1, oR1, sel), __byte_perm(I1, oI1, sel));   // thread tid0 + 2
             }
         }
-        __syncthreads();
+        // ---- the segments of this template (one pass; more with bfly_correlate_multi).  The barrier
+        //      at the head of a pass is "G is in place" for the first and the segment boundary for the
+        //      others (ptxas needs a barrier between the divergent end of a pass and the block loop
+        //      to keep that loop on the uniform datapath).
+        int sg = 0;
         float thr = 0.0f, rsig2 = 0.0f;               // TAILS: kappa^2 sigma^2 / inc2 and inc2 / sigma^2
+        do {
+        __syncthreads();
         if (TAILS) {
             float acc = 0.0f;
 #pragma unroll
@@ -605,8 +634,10 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             wb = wb + 1 == N_EXCH ? 0 : wb + 1;
         };
 
+        const float4 *rn2p_s = MULTI ? rn2p + (int64_t)sg * n_blocks * (NT * 2) : rn2p;
+        const float *rn2_s = MULTI ? sa.rn2[sg] : rn2;
         float best = -1.0f;
-        int32_t code = 0;                              // 8 b + 2 i + e
+        int32_t code = 0;                              // 8 b + 4 e + i
         if (n_blocks > 0) front();
         for (int32_t b = 0; b < n_blocks; ++b) {
             mbar_wait(sm.bar + rb, (fpar >> rb) & 1);
@@ -617,7 +648,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 mbar_expect_tx(sm.bar + 3 + slot, XB_BYTES);
                 bulk_load(sm.xs + slot * (EXCH_WORDS / 4), xh + (int64_t)next_b * (EXCH_WORDS / 4), XB_BYTES,
                           sm.bar + 3 + slot);
-                next_b = next_b + 1 == n_blocks ? 0 : next_b + 1;
+                next_b = next_b + 1 == seq_blocks ? 0 : next_b + 1;
                 ++issued;
                 // The next template's parameters (cp.async of thread 0, issued a whole G stage ago:
                 // this wait does not stall) become visible to every warp through thread 0's arrivals
@@ -627,13 +658,13 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             }
             const uint4 *rbuf = sm.exch + rb * (EXCH_WORDS / 4);
             rb = rb + 1 == N_EXCH ? 0 : rb + 1;
-            // ---- the two halves of an iteration, passes A, B of block b + 1 ("front") and passes C, D
-            //      + A5-A7 of block b ("back"), are independent; half of the warps of every scheduler
-            //      (w >> 3) run them in the other order, so that the tensor-pipe bursts of one half
-            //      fall on the FMA / ALU bursts of the other (measured: DESIGN.md 10)
+            // ---- the two halves of an iteration: passes A, B of block b + 1 ("front"), then passes
+            //      C, D + A5-A7 of block b ("back").  (Running them in the other order in half of the
+            //      warps of every scheduler, so that tensor-pipe bursts meet FMA bursts, was measured
+            //      slower: DESIGN.md 10.)
             auto back = [&]() {
                 // ---- passes C, D and A5-A7 on the 8 lags of this thread
-                const float4 *rp = rn2p + ((int64_t)b * NT + tid) * 2;
+                const float4 *rp = rn2p_s + ((int64_t)b * NT + tid) * 2;
                 const float4 ra = __ldg(rp), rb4 = __ldg(rp + 1);
                 const float2 rr[4] = {make_float2(ra.x, ra.y), make_float2(ra.z, ra.w),
                                       make_float2(rb4.x, rb4.y), make_float2(rb4.z, rb4.w)};
@@ -648,43 +679,18 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                         qs4[i] = q;
                         qmax = fmaxf(qmax, fmaxf(q.x, q.y));
                     } else {
-#if BFLY_TC_EPI == 2
-                        // A7 inside the thread: the low three mantissa bits of q (2^-21 relative, far
-                        // below the fp16 operand noise) carry 7 - (rank of the lag among the thread's
-                        // eight lags of this block: lag = .. + i + 64 e, so rank = 4 e + i): the
-                        // largest key is the largest q and, on a tie, the smallest lag (reading C8).
-                        // NaN (0 x -inf past the last lag) and -inf keys never win a maximum.
-                        qs4[i].x = __uint_as_float((__float_as_uint(q.x) & 0xFFFFFFF8u) | (uint32_t)(7 - i));
-                        qs4[i].y = __uint_as_float((__float_as_uint(q.y) & 0xFFFFFFF8u) | (uint32_t)(3 - i));
-#elif BFLY_TC_EPI == 1
                         // A7 inside the thread, in lag order (reading C8: ties to the smallest lag): the
                         // thread's lags of this block are .. + i + 64 e, so the e = 0 lags are compared
                         // here and the e = 1 lags after the loop; code = 8 b + 4 e + i
                         if (q.x > best) { best = q.x; code = 8 * b + i; }
                         qs4[i].y = q.y;
-#else
-                        if (q.x > best) { best = q.x; code = 8 * b + i; }
-                        if (q.y > best) { best = q.y; code = 8 * b + 4 + i; }
-#endif
                     }
                 }
-#if BFLY_TC_EPI == 2
-                if (!TAILS) {
-                    const float bm = fmaxf(fmaxf(fmaxf(qs4[0].x, qs4[1].x), fmaxf(qs4[2].x, qs4[3].x)),
-                                           fmaxf(fmaxf(qs4[0].y, qs4[1].y), fmaxf(qs4[2].y, qs4[3].y)));
-                    // `best` keeps its low bits at 7, so a later block wins only with a larger q
-                    if (bm > best) {
-                        best = __uint_as_float(__float_as_uint(bm) | 7u);
-                        code = 8 * b + 7 - (int32_t)(__float_as_uint(bm) & 7u);
-                    }
-                }
-#elif BFLY_TC_EPI == 1
                 if (!TAILS) {
 #pragma unroll
                     for (int i = 0; i < 4; ++i)
                         if (qs4[i].y > best) { best = qs4[i].y; code = 8 * b + 4 + i; }
                 }
-#endif
                 if (TAILS && qmax > thr) {                 // rare: at least one of this thread's 8 lags is a hit
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
@@ -702,27 +708,9 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                         }
                     }
                 }
-        
             };
-#if BFLY_TC_DEPHASE
-            if (w & 8) {
-                back();
-                if (b + 1 < n_blocks) front();
-            } else
-#endif
-            {
-#if BFLY_TC_PEEL
-                if (b + 1 < n_blocks) {                // one straight-line stretch: the scheduler may interleave the two
-                    front();
-                    back();
-                } else {
-                    back();
-                }
-#else
-                if (b + 1 < n_blocks) front();
-                back();
-#endif
-            }
+            if (b + 1 < n_blocks) front();
+            back();
         }
         // ---- tail lags from the transform of the last block: lag n_blocks TCV + r is its output
         //      n = 4096 + r, i.e. row delta = 8 of the last pass (the rows chain2<FULL> adds) of unit
@@ -735,7 +723,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             for (int h = 0; h < 2; ++h)
 #pragma unroll
                 for (int q = 0; q < 3; ++q) w16u[h][q] = sm.w16u[(h * 3 + q) * 32 + lane];
-            const float qsl = (float)__ldg(qs + (n_blocks - 1));
+            const float qsl = (float)__ldg(qs + ((MULTI ? sg * n_blocks : 0) + n_blocks - 1));
 #pragma unroll 1
             for (int r = 0; r < n_ftail; ++r) {
                 cpair z, zu;
@@ -752,7 +740,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                             }
                         }
                     } else {
-                        const float q = m2 * __ldg(rn2 + (int64_t)n_blocks * TCV + r);
+                        const float q = m2 * __ldg(rn2_s + (int64_t)n_blocks * TCV + r);
                         if (q > best) { best = q; code = 8 * n_blocks + r; }
                     }
                 }
@@ -777,18 +765,9 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     }
                 }
             } else {
-                const float q = fmaf(s, s, c * c) * __ldg(rn2 + (int64_t)n_blocks * TCV + tid);
-#if BFLY_TC_EPI == 2
-                const float qt = __uint_as_float(__float_as_uint(q) & 0xFFFFFFF8u);
-                if (qt > best) { best = __uint_as_float(__float_as_uint(qt) | 7u); code = 8 * n_blocks + tid; }
-#else
+                const float q = fmaf(s, s, c * c) * __ldg(rn2_s + (int64_t)n_blocks * TCV + tid);
                 if (q > best) { best = q; code = 8 * n_blocks + tid; }
-#endif
             }
-        }
-        if (n_blocks < 2) {                            // too few block iterations to publish the parameters through
-            if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
-            __syncthreads();
         }
         if (!TAILS) {
             unsigned long long p = 0ull;
@@ -797,18 +776,19 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * TCV + (uint32_t)(code - 8 * n_blocks)
                                                    : (uint32_t)bb * TCV + (uint32_t)((4 * w + (rank & 3)) +
                                                                                      64 * (2 * t + (rank >> 2)) + 512 * g);
-#if BFLY_TC_EPI == 2
-                p = ((unsigned long long)(__float_as_uint(best) & 0xFFFFFFF8u) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
-#else
                 p = ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
-#endif
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 const unsigned long long q = __shfl_xor_sync(0xffffffffu, p, o);
                 p = q > p ? q : p;
             }
-            if (lane == 0) sm.red[16 * ps + w] = p;    // combined by thread 0 after the next template's first barrier
+            if (lane == 0) sm.red[16 * ((MULTI ? MAX_SEG : 1) * ps + sg) + w] = p;   // combined by thread 0 after the next template's first barrier
+        }
+        } while (MULTI && ++sg < n_seg);               // segments
+        if (seq_blocks < 2) {                          // too few block iterations to publish the parameters through
+            if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();
         }
     }
     if (!TAILS && blockIdx.x < T) {
@@ -879,20 +859,42 @@ static int tc_attrs(int device)
     return once.run(device, []() -> int {
         BFLY_CUDA(cudaFuncSetAttribute(tc_spectra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_wspec_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft32::FFT_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
-        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<false, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+        BFLY_CUDA(cudaFuncSetAttribute(tc_correlate_kernel<true, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         BFLY_CUDA(cudaFuncSetAttribute(tc_debug_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
         return BFLY_OK;
     });
 }
 
-static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
-                            int64_t lag_end, float *rho_max, int32_t *arg_lag, const TailArgs *tails,
-                            cudaStream_t stream)
+// Whether the lags past the last whole block come from the last block's transform: output
+// n = 4096 + r of that transform is a valid (unwrapped) lag while 4096 + r <= B - L; then the kernel
+// takes them from the rows delta >= 8 (n_ftail) and the synthesis carries no direct sums.
+static bool tail_from_transform(int32_t L, int64_t n_blocks, int32_t n_tail)
+{
+    return n_tail > 0 && n_blocks > 0 && (int64_t)(n_tail - 1) <= (int64_t)TCV - (int64_t)L;
+}
+
+// Several equal-length segments in one launch need every lag to come from a transform.
+bool tc_multi_supported(int32_t L, int64_t n_lags)
+{
+    int64_t nb; int32_t nt;
+    tc_plan(n_lags, &nb, &nt);
+    return L >= BFLY_TC_MIN_L && nb > 0 && (nt == 0 || tail_from_transform(L, nb, nt));
+}
+
+// n_seg segments x[s] of n_samples samples each, the same lag range in each; rn2 of segment s at
+// b->rn2 + s n_lags (written by the caller); spectra, scales and normalisers of segment s occupy
+// blocks s n_blocks .. of the bank's workspace.
+static int launch_tc_common(const bfly_bank *b, int n_seg, const float *const *x, int64_t n_samples,
+                            int64_t lag_begin, int64_t lag_end, float *const *rho_max, int32_t *const *arg_lag,
+                            const TailArgs *tails, cudaStream_t stream)
 {
     int rc = tc_attrs(b->device);
     if (rc) return rc;
@@ -900,42 +902,59 @@ static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_sample
     if (n_lags >= (1LL << 31) - 2 * TCV) { set_error("too many lags"); return BFLY_ERANGE; }
     int64_t n_blocks; int32_t n_tail;
     tc_plan(n_lags, &n_blocks, &n_tail);
-    if (n_blocks * 2 * EXCH_WORDS > b->xh_cap || n_blocks * TCV > b->rn2p_cap) {
+    if (n_seg < 1 || n_seg > MAX_SEG || (n_seg > 1 && (tails || !tc_multi_supported(b->L, n_lags)))) {
+        set_error("unsupported multi-segment launch (internal)");
+        return BFLY_EINVAL;
+    }
+    if (n_seg * n_blocks * 2 * EXCH_WORDS > b->xh_cap || n_seg * n_blocks * TCV > b->rn2p_cap ||
+        n_seg * n_blocks > b->qs_cap || (n_seg > 1 && n_seg * n_lags > b->rn2_cap)) {
         set_error("FFT workspace too small (internal)");
         return BFLY_EINVAL;
     }
     if (n_blocks > 0) {
-        tc_spectra_kernel<<<(unsigned)n_blocks, fft32::NT, fft32::FFT_SMEM, stream>>>(
-            x, n_samples, lag_begin, b->xh, b->qs);
-        count_launch();
-        BFLY_CUDA(cudaGetLastError());
-        const int64_t n_slots = n_blocks * TCV;
-        tc_norm_kernel<<<(unsigned)((n_slots + 255) / 256), 256, 0, stream>>>(
-            x, b->L, lag_begin, n_lags - n_tail, b->qs, b->rn2p, n_slots, tails ? 1 : 0);
-        count_launch();
-        BFLY_CUDA(cudaGetLastError());
+        for (int sg = 0; sg < n_seg; ++sg) {
+            tc_spectra_kernel<<<(unsigned)n_blocks, fft32::NT, fft32::FFT_SMEM, stream>>>(
+                x[sg], n_samples, lag_begin, b->xh + (int64_t)sg * n_blocks * 2 * EXCH_WORDS, b->qs + sg * n_blocks);
+            count_launch();
+            BFLY_CUDA(cudaGetLastError());
+            const int64_t n_slots = n_blocks * TCV;
+            tc_norm_kernel<<<(unsigned)((n_slots + 255) / 256), 256, 0, stream>>>(
+                x[sg], b->L, lag_begin, n_lags - n_tail, b->qs + sg * n_blocks, b->rn2p + (int64_t)sg * n_slots, n_slots,
+                tails ? 1 : 0);
+            count_launch();
+            BFLY_CUDA(cudaGetLastError());
+        }
     }
     const int64_t ctas = b->T < (int64_t)b->sm_count ? b->T : (int64_t)b->sm_count;
-    // The lags past the last whole block: output n = 4096 + r of the last block's transform is
-    // a valid (unwrapped) lag while 4096 + r <= B - L; then the kernel takes them from the rows
-    // delta >= 8 of that transform (n_ftail) and the synthesis carries no direct sums (n_dtail).
-    const bool tail_by_fft = n_tail > 0 && n_blocks > 0 && (int64_t)(n_tail - 1) <= (int64_t)TCV - (int64_t)b->L;
+    const bool tail_by_fft = tail_from_transform(b->L, n_blocks, n_tail);
     const int32_t n_ftail = tail_by_fft ? n_tail : 0, n_dtail = tail_by_fft ? 0 : n_tail;
+    SegArgs sa{};
+    sa.n_seg = n_seg;
+    for (int sg = 0; sg < n_seg; ++sg) {
+        sa.rn2[sg] = b->rn2 + (int64_t)sg * n_lags;
+        sa.lag_begin[sg] = lag_begin;
+        sa.rho_max[sg] = rho_max ? rho_max[sg] : nullptr;
+        sa.arg_lag[sg] = arg_lag ? arg_lag[sg] : nullptr;
+    }
     core_timer_start(b, stream);
-#define BFLY_TC_LAUNCH(TAILS_, FAM_, ARGS_)                                                            \
-    tc_correlate_kernel<TAILS_, FAM_><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(                        \
+#define BFLY_TC_LAUNCH(TAILS_, FAM_, MULTI_, ARGS_)                                                    \
+    tc_correlate_kernel<TAILS_, FAM_, MULTI_><<<(unsigned)ctas, NT, TC_SMEM, stream>>>(                \
         b->T, b->L, b->phA, b->phB, b->phC, b->inc2, b->ins2, reinterpret_cast<const uint4 *>(b->xh), \
-        reinterpret_cast<const float4 *>(b->rn2p), x, b->rn2, lag_begin, (int32_t)n_blocks, n_dtail,   \
-        n_ftail, b->qs, rho_max, arg_lag, ARGS_)
+        reinterpret_cast<const float4 *>(b->rn2p), x[0], b->rn2, lag_begin, (int32_t)n_blocks, n_dtail, \
+        n_ftail, b->qs, sa.rho_max[0], sa.arg_lag[0], sa, ARGS_)
     const int fam = b->family == BFLY_FAMILY_SETTLE ? 2 : b->has_f2 ? 1 : 0;
     if (tails) {
-        if (fam == 2) BFLY_TC_LAUNCH(true, 2, *tails);
-        else if (fam == 1) BFLY_TC_LAUNCH(true, 1, *tails);
-        else BFLY_TC_LAUNCH(true, 0, *tails);
+        if (fam == 2) BFLY_TC_LAUNCH(true, 2, false, *tails);
+        else if (fam == 1) BFLY_TC_LAUNCH(true, 1, false, *tails);
+        else BFLY_TC_LAUNCH(true, 0, false, *tails);
+    } else if (n_seg > 1) {
+        if (fam == 2) BFLY_TC_LAUNCH(false, 2, true, TailArgs{});
+        else if (fam == 1) BFLY_TC_LAUNCH(false, 1, true, TailArgs{});
+        else BFLY_TC_LAUNCH(false, 0, true, TailArgs{});
     } else {
-        if (fam == 2) BFLY_TC_LAUNCH(false, 2, TailArgs{});
-        else if (fam == 1) BFLY_TC_LAUNCH(false, 1, TailArgs{});
-        else BFLY_TC_LAUNCH(false, 0, TailArgs{});
+        if (fam == 2) BFLY_TC_LAUNCH(false, 2, false, TailArgs{});
+        else if (fam == 1) BFLY_TC_LAUNCH(false, 1, false, TailArgs{});
+        else BFLY_TC_LAUNCH(false, 0, false, TailArgs{});
     }
 #undef BFLY_TC_LAUNCH
     core_timer_stop(b, stream);
@@ -947,7 +966,13 @@ static int launch_tc_common(const bfly_bank *b, const float *x, int64_t n_sample
 int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                   int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream)
 {
-    return launch_tc_common(b, x, n_samples, lag_begin, lag_end, rho_max, arg_lag, nullptr, stream);
+    return launch_tc_common(b, 1, &x, n_samples, lag_begin, lag_end, &rho_max, &arg_lag, nullptr, stream);
+}
+
+int launch_fft_tc_multi(const bfly_bank *b, int n_seg, const float *const *x, int64_t n_samples, int64_t lag_begin,
+                        int64_t lag_end, float *const *rho_max, int32_t *const *arg_lag, cudaStream_t stream)
+{
+    return launch_tc_common(b, n_seg, x, n_samples, lag_begin, lag_end, rho_max, arg_lag, nullptr, stream);
 }
 
 // bfly_tails: predictor step (autocorrelation of the segment, its transform W), then the
@@ -975,7 +1000,7 @@ int launch_tails_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64
     ta.hit_lag = hit_lag;
     ta.hit_rho = hit_rho;
     ta.n_hits = n_hits;
-    return launch_tc_common(b, x, n_samples, lag_begin, lag_end, nullptr, nullptr, &ta, stream);
+    return launch_tc_common(b, 1, &x, n_samples, lag_begin, lag_end, nullptr, nullptr, &ta, stream);
 }
 
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream)

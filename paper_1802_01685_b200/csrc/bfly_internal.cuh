@@ -52,6 +52,9 @@ struct bfly_bank {
     unsigned long long *packed;  // T packed (rho^2 bits, ~lag) words for the direct form
     float *x_stage;           // device copy of a host chunk (bfly_search_host)
     int64_t x_stage_cap;
+    float *rho_multi;         // bfly_search_host with several chunks per launch: group x T each
+    int32_t *arg_multi;
+    int64_t rho_multi_cap, arg_multi_cap;
     float *rho_stage;         // T
     int32_t *arg_stage;       // T
     uint32_t *map_stage;
@@ -164,6 +167,9 @@ int64_t fft_blocks_needed(int32_t L, int64_t n_lags);
 int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                   int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int64_t tc_blocks_needed(int64_t n_lags);
+bool tc_multi_supported(int32_t L, int64_t n_lags);
+int launch_fft_tc_multi(const bfly_bank *b, int n_seg, const float *const *x, int64_t n_samples, int64_t lag_begin,
+                        int64_t lag_end, float *const *rho_max, int32_t *const *arg_lag, cudaStream_t stream);
 void tc_plan(int64_t n_lags, int64_t *n_blocks, int32_t *n_tail);
 int launch_fft_tc5(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                    int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);

@@ -482,3 +482,31 @@ def test_determinism_soak_at_ragged_sizes(bfly, form, N):
     idx = np.array([0, 147, 148, 2000, T - 1])
     f0, f1, _, _ = bank.get()
     check_values_and_argmax(x.cpu().numpy(), fs, L, f0[idx], f1[idx], r0.cpu().numpy()[idx], a0.cpu().numpy()[idx])
+
+
+# ----------------------------------------------------------------- several segments per launch
+@pytest.mark.parametrize("fs,L,N,S", [(4096.0, 4096, 65536, 2), (4096.0, 4096, 36864, 4), (2048.0, 2048, 20000, 3),
+                                       (1000.0, 300, 9000, 5), (4096.0, 4096, 4096 * 3 + 2, 2), (4096.0, 4096, 6000, 2)])
+def test_correlate_multi_equals_one_call_per_segment(bfly, fs, L, N, S):
+    """bfly_correlate_multi (the same bank on two detectors; chunks of a stream):
+    synthesis and the transform of g once per template for up to four segments.  Its results are
+    those of one bfly_correlate per segment, bit for bit; the first segment is also checked against
+    the oracle.  Shapes: config-4-sized segments, a ragged last block, five segments (4 + 1), one
+    whose last lags are direct sums (falls back to one call per segment), one shorter than a block."""
+    rng = np.random.default_rng(int(N) + S)
+    T = 148 + 23
+    f0 = rng.uniform(0.05 * fs, 0.45 * fs, T)
+    f1 = rng.uniform(-0.2 * fs, 0.2 * fs, T)
+    bank = bfly.make_bank(fs, L, f0, f1)
+    xs = [rng.standard_normal(N).astype(np.float32) * np.float32(10.0 ** rng.integers(-2, 3)) for _ in range(S)]
+    hc, _ = oracle.template(fs, L, f0[5], f1[5])
+    xs[-1][100:100 + L] += np.float32(0.4 * np.std(xs[-1])) * hc.astype(np.float32)
+    xd = [torch.from_numpy(x).cuda() for x in xs]
+    for lb, le in ((0, None), (17, min(N - L + 1, 17 + 4096 + 1))):
+        rho_m, arg_m = bfly.correlate_multi(bank, xd, lb, le)
+        torch.cuda.synchronize()
+        for s in range(S):
+            rho_1, arg_1 = bfly.correlate(bank, xd[s], lb, le)
+            torch.cuda.synchronize()
+            assert torch.equal(rho_m[s], rho_1) and torch.equal(arg_m[s], arg_1), (s, lb, le)
+        check_values_and_argmax(xs[0], fs, L, f0, f1, rho_m[0].cpu().numpy(), arg_m[0].cpu().numpy(), lb, le)
