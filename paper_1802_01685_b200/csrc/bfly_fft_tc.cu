@@ -226,11 +226,13 @@ __device__ __forceinline__ void synth_sincos(uint32_t Ahi, uint32_t Alo, uint32_
 }
 
 // Where thread `th`'s 16-byte operand chunk of G sits inside a 512-chunk row of sm.gs: bit 3 of the
-// thread index folded into bit 1.  The lanes of a warp that store G (transform output order) differ
-// in bits 0, 2, 3, 4, 8 of the owning thread's index, so without the fold they hit 4 of the 8
-// 16-byte bank groups (ncu: 16 wavefronts per 8-byte store instead of 4); the readers' lanes
-// differ in bits 0-4, of which the fold keeps bits 0-2 a permutation: still conflict free.
-__device__ __forceinline__ int gs_slot(int th) { return th ^ ((th >> 2) & 2); }
+// thread index folded into bit 1 and bit 4 into bit 0.  The lanes of a warp that store G
+// (transform output order) differ in bits 0, 2, 3, 4, 8 of the owning thread's index -- and the
+// lanes of a half-warp in bits 2, 3, 4, 8 only --, so without the folds they hit 4 (2) of the 8
+// 16-byte bank groups: ncu showed 16 wavefronts per 8-byte store with no fold, 8 with the first
+// fold alone, 4 is the minimum (every lane writes the same half of its chunk).  The readers' lanes
+// differ in bits 0-4, of which the folds keep bits 0-2 a permutation: still conflict free.
+__device__ __forceinline__ int gs_slot(int th) { return th ^ ((th >> 2) & 2) ^ ((th >> 4) & 1); }
 
 // Index of tail-window sample n in sm.xt: a thread's lanes differ in bits 7-9 (g) and 11-12 (t)
 // of n; folding those into the bank bits makes the reads conflict free.
