@@ -14,6 +14,8 @@
 // Data scaling: every block of x is multiplied by a power of two that puts its rms in [1, 2)
 // (rho is scale invariant), so all intermediates sit well inside the fp16 range; the factor is
 // folded, in float64, into the per-lag normaliser tc_norm_kernel writes.
+#include <type_traits>
+
 #include "bfly_fft32.cuh"
 #include "bfly_fft_tc.cuh"
 
@@ -468,6 +470,9 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             for (int r = 0; r < MAX_TAIL; ++r) tc_[r] = ts_[r] = 0.0f;
             const int to = pt & 1, uh = pt >> 1;
             uint32_t pr[4], pi[4];
+            // (templates of the full 4096 samples -- every config but one -- need no n < L test: a
+            // uniform branch picks the instantiation without it)
+            auto synth = [&](auto checked) {
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
                 const int c = 4 * (pw >> 3) + 2 * uh + (kk >> 1), dp = (pw & 7) + 8 * (kk & 1);
@@ -476,7 +481,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 for (int e = 0; e < 2; ++e) {
                     const int n = 1024 * (2 * to + e) + 128 * pg + 16 * c + dp;
                     cs[e] = sn[e] = 0.0f;
-                    if (n < L) {
+                    if (!decltype(checked)::value || n < L) {
                         if (FAM == 0) {              // linear chirp
                             synth_sincos(Ahi, Alo, Bhi, Blo, (uint32_t)n, &sn[e], &cs[e]);
                         } else {                     // N1: cubic phase, full 64-bit Horner; N2: settling
@@ -507,6 +512,9 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 pr[kk] = pack_h2(cs[0], cs[1]);
                 pi[kk] = pack_h2(-sn[0], -sn[1]);
             }
+            };
+            if (L == FFT_MAX_L) synth(std::false_type{});
+            else synth(std::true_type{});
             const bool owner = pt < 2;
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
