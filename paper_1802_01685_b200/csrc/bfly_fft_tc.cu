@@ -185,10 +185,12 @@ struct TcSmem {
     uint32_t *w16u;            // [2][3][32]: A fragments of W16 rows 8..15 (G transform only)
     float *tail;               // [2][16 warps][2 MAX_TAIL] partial sums of the direct tail lags
     unsigned long long *red;   // [2][16]
+    float *icv;                // [2]: inc2 of the template whose maxima sit in red[parity] (for write_out)
     unsigned char *par;        // [2][32]: {phA, phB, phC, inc2, ins2} of the template after this one
     unsigned long long *bar;   // mbarriers: [0..2] exchange buffer full, [3..4] X_b slot filled
 };
 constexpr int N_EXCH = 3;
+constexpr int OUT_TID = 12 * 32;                             // the thread that combines and writes a template's outputs
 constexpr size_t OFF_GS = (size_t)N_EXCH * EXCH_WORDS * 4;
 constexpr size_t OFF_XS = OFF_GS + EXCH_WORDS * 4;
 constexpr size_t OFF_XT = OFF_XS + 2 * EXCH_WORDS * 4;
@@ -197,7 +199,8 @@ constexpr size_t OFF_TAIL = OFF_W16U + 2 * 3 * 32 * 4;
 constexpr size_t OFF_RED = OFF_TAIL + 2 * 16 * 2 * MAX_TAIL * 4;   // tail[] is double buffered by template parity
 constexpr size_t OFF_BAR = OFF_RED + 2 * 4 * 16 * 8;          // red[parity][segment][warp]
 constexpr size_t OFF_PAR = OFF_BAR + 8 * 8;                   // two slots of prefetched bank parameters
-constexpr size_t TC_SMEM = OFF_PAR + 2 * 32;
+constexpr size_t OFF_ICV = OFF_PAR + 2 * 32;                 // 1 / ||cos phi||^2 of the two templates in flight
+constexpr size_t TC_SMEM = OFF_ICV + 16;
 __device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
 {
     TcSmem s;
@@ -210,6 +213,7 @@ __device__ __forceinline__ TcSmem carve_tc(unsigned char *base)
     s.red = reinterpret_cast<unsigned long long *>(base + OFF_RED);
     s.bar = reinterpret_cast<unsigned long long *>(base + OFF_BAR);
     s.par = base + OFF_PAR;
+    s.icv = reinterpret_cast<float *>(base + OFF_ICV);
     return s;
 }
 
@@ -410,13 +414,13 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 rho_max[jo] = 0.0f;
                 arg_lag[jo] = (int32_t)lag_begin;
             } else {
-                const float ico = *reinterpret_cast<const float *>(sm.par + 32 * slot + 24);
+                const float ico = sm.icv[slot];
                 rho_max[jo] = sqrtf(__uint_as_float((uint32_t)(p >> 32)) * ico);
                 arg_lag[jo] = (int32_t)(lag_begin + (int64_t)(0xFFFFFFFFu - (uint32_t)(p & 0xFFFFFFFFull)));
             }
             return;
         }
-        const float ico = *reinterpret_cast<const float *>(sm.par + 32 * slot + 24);
+        const float ico = sm.icv[slot];
         for (int sg = 0; sg < n_seg; ++sg) {
             const unsigned long long *red = sm.red + 16 * (MAX_SEG * slot + sg);
             unsigned long long p = red[0];
@@ -449,7 +453,8 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         const uint32_t Ahi = (uint32_t)(A >> 32), Alo = (uint32_t)A;
         const uint32_t Bhi = (uint32_t)(Bq >> 32), Blo = (uint32_t)Bq;
         const float ic = *reinterpret_cast<const float *>(pp + 24);
-        const float rq = sqrtf(*reinterpret_cast<const float *>(pp + 28) / ic);   // ic > 0: cos phi_0 = 1
+        // ic > 0 (cos phi_0 = 1); fast division and square root: r enters g before its fp16 rounding
+        const float rq = __fsqrt_rn(__fdividef(*reinterpret_cast<const float *>(pp + 28), ic));
         // The index arithmetic of the per-template code below depends on the thread only, so the
         // compiler would hoist it out of the template loop and hold its results in registers all
         // through the block loop -- which is at the 128-register limit and then recomputes its OWN
@@ -544,10 +549,10 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             chain1(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
         }
         __syncthreads();                                // every warp has left the previous template
-        if (tid == 0) {
-            if (!TAILS && j != (int64_t)blockIdx.x) write_out(j - gridDim.x, ps ^ 1);
-            if (j + gridDim.x < T) prefetch_params(j + gridDim.x, ps ^ 1);     // after write_out: it reads that slot's inc2
-        }
+        // (the per-template chores are spread over warps 0, 8 and 12 so that no warp trails the others
+        // into the next barrier: thread 0 owns the copies, OUT_TID the outputs, warp 8 the tail lags)
+        if (tid == OUT_TID && !TAILS && j != (int64_t)blockIdx.x) write_out(j - gridDim.x, ps ^ 1);
+        if (tid == 0 && j + gridDim.x < T) prefetch_params(j + gridDim.x, ps ^ 1);
         // ---- G = F+(g): all 16 rows of the last pass; G / S16 -> fp16 -> operand layout
         {
             uint32_t w16u[2][3];
@@ -724,9 +729,9 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         }
         // ---- tail lags from the transform of the last block: lag n_blocks TCV + r is its output
         //      n = 4096 + r, i.e. row delta = 8 of the last pass (the rows chain2<FULL> adds) of unit
-        //      U = r, which belongs to warp 0 -- lane 0 holds (gamma, delta) = (0, 8).  That buffer
+        //      U = r (any warp can run it: warp 8 does) -- lane 0 holds (gamma, delta) = (0, 8).  That buffer
         //      is intact: the next writers of it are two transforms away, behind the next barrier.
-        if (n_ftail > 0 && w == 0) {
+        if (n_ftail > 0 && w == 8) {
             const uint4 *lbuf = sm.exch + (rb == 0 ? N_EXCH - 1 : rb - 1) * (EXCH_WORDS / 4);
             uint32_t w16u[2][3];
 #pragma unroll
@@ -793,9 +798,10 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 const unsigned long long q = __shfl_xor_sync(0xffffffffu, p, o);
                 p = q > p ? q : p;
             }
-            if (lane == 0) sm.red[16 * ((MULTI ? MAX_SEG : 1) * ps + sg) + w] = p;   // combined by thread 0 after the next template's first barrier
+            if (lane == 0) sm.red[16 * ((MULTI ? MAX_SEG : 1) * ps + sg) + w] = p;   // combined by OUT_TID after the next template's first barrier
         }
         } while (MULTI && ++sg < n_seg);               // segments
+        if (!TAILS && tid == 0) sm.icv[ps] = *reinterpret_cast<const float *>(sm.par + 32 * ps + 24);
         if (seq_blocks < 2) {                          // too few block iterations to publish the parameters through
             if (tid == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncthreads();
@@ -803,7 +809,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
     }
     if (!TAILS && blockIdx.x < T) {
         __syncthreads();
-        if (tid == 0) write_out(j - gridDim.x, ps ^ 1);
+        if (tid == OUT_TID) write_out(j - gridDim.x, ps ^ 1);
     }
 }
 
