@@ -270,9 +270,12 @@ __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
         "WAIT_DONE:\n"
         "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
 }
+// (No proxy fence: the destination slot was only READ through the generic proxy, and those reads
+// are ordered before this copy by the mbarrier the issuing thread has waited on -- the
+// consumer-release / producer-acquire pattern of every TMA pipeline.  fence.proxy.async is for
+// generic WRITES that the async proxy must see; here it cost warp 0 a MEMBAR.ALL.CTA per block.)
 __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, void *bar)
 {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
 }
