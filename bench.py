@@ -453,6 +453,24 @@ def main():
                                 "note": "the same overlap-save FFT with the length-8192 transform as 64 x 128 on "
                                         "tcgen05.mma (DFT matrices in tensor memory); measured slower than the "
                                         "mma.sync transform (DESIGN.md 10), hence not the default"}
+            # several segments per launch (bfly_correlate_multi: the two detectors of PAPER.md:124, the
+            # chunks of a stream): two 16-s segments through one launch against one call each
+            x2 = torch.flip(xd, dims=[0]).contiguous()
+            def _ms(fn, reps=3):
+                fn(); torch.cuda.synchronize()
+                a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a0.record()
+                for _ in range(reps):
+                    fn()
+                a1.record(); torch.cuda.synchronize()
+                return a0.elapsed_time(a1) / reps
+            t_multi = _ms(lambda: bfly.correlate_multi(dbank, [xd, x2]))
+            t_each = _ms(lambda: (bfly.correlate(dbank, xd), bfly.correlate(dbank, x2)))
+            other["multi_segment"] = {"kernel": "tc_correlate_kernel<MULTI>", "templates": nd, "segments": 2,
+                                      "ms_one_launch": t_multi, "ms_one_call_each": t_each,
+                                      "value": 2 * correlations_per_step(cfg, nd) / (t_multi * 1e-3), "unit": UNIT,
+                                      "note": "synthesis and the transform of g once per template for both segments; "
+                                              "results bit-identical to one call per segment"}
             # the paper's own reduction on the same kernel: sigma by Parseval + all tails above
             # kappa sigma (bfly_tails), whole bank, kappa = 5.5 (about 1e5 hits in noise)
             bank.set_timing(True)

@@ -388,6 +388,8 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                       sm.bar + 3 + (int)issued);
             next_b = next_b + 1 == seq_blocks ? 0 : next_b + 1;
         }
+    int gs_tid = gs_slot(tid);                         // held in a register: recomputing it costs the block loop two instructions
+    asm volatile("" : "+r"(gs_tid));
     uint32_t xcnt = 0;                                 // blocks consumed: slot = xcnt & 1, parity = (xcnt >> 1) & 1
     int wb = 0, rb = 0;                                // exchange buffer written next / read next
     uint32_t fpar = 0;                                 // bit i: parity to wait for on "full(i)"
@@ -637,7 +639,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 #pragma unroll
             for (int ci = 0; ci < 4; ++ci) {
                 const uint4 xq = xb[ci * NT];
-                const uint4 gq = sm.gs[ci * NT + gs_slot(tid)];
+                const uint4 gq = sm.gs[ci * NT + gs_tid];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const __half2 xr = as_h2(h ? xq.z : xq.x), xi = as_h2(h ? xq.w : xq.y);
