@@ -659,6 +659,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
 
         const float4 *rn2p_s = MULTI ? rn2p + (int64_t)sg * n_blocks * (NT * 2) : rn2p;
         const float *rn2_s = MULTI ? sa.rn2[sg] : rn2;
+        const float4 *rp_run = rn2p_s + tid * 2;       // MULTI: this thread's normalisers, block by block
         float best = -1.0f;
         int32_t code = 0;                              // 8 b + 4 e + i
         if (n_blocks > 0) front();
@@ -687,7 +688,8 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
             //      slower: DESIGN.md 10.)
             auto back = [&]() {
                 // ---- passes C, D and A5-A7 on the 8 lags of this thread
-                const float4 *rp = rn2p_s + ((int64_t)b * NT + tid) * 2;
+                const float4 *rp = MULTI ? rp_run : rn2p_s + ((int64_t)b * NT + tid) * 2;
+                if (MULTI) rp_run += NT * 2;
                 const float4 ra = __ldg(rp), rb4 = __ldg(rp + 1);
                 const float2 rr[4] = {make_float2(ra.x, ra.y), make_float2(ra.z, ra.w),
                                       make_float2(rb4.x, rb4.y), make_float2(rb4.z, rb4.w)};
