@@ -171,6 +171,27 @@ int bfly_correlate(const bfly_bank *bank, const float *x_dev, int64_t n_samples,
                    int64_t lag_begin, int64_t lag_end,
                    float *rho_max_dev, int32_t *arg_lag_dev, void *stream);
 
+/* ---- the same without any allocation -------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it): bfly_correlate in its default form (BFLY_FORM_FFT_TC: needs
+ * L >= BFLY_TC_MIN_L, else BFLY_EUNSUPPORTED) with the per-call scratch -- data-block spectra,
+ * per-lag normalisers, block scales: what bfly_correlate keeps in the bank's workspace -- in a
+ * file-scope static device array of 1 MB + 256 B inside the library, which every GPU that loads
+ * the library holds until the process exits.  Arguments, layouts, results (bit for bit) and error
+ * behaviour as bfly_correlate (rows A2-A7), except:
+ *  - n_samples <= BFLY_STATIC_MAX_SAMPLES (one 16-s segment at 4096 Hz, 16 overlap-save blocks);
+ *    a longer segment returns BFLY_ERANGE and launches nothing;
+ *  - the call allocates and frees nothing, on the host or the device, reads the bank's
+ *    parameters only, does not touch its workspace and does not take its in-use flag;
+ *  - ALL calls, on any bank and any stream of the same device, share the one array: two calls
+ *    that overlap on the GPU race (serialise them on one stream or with events).  The array
+ *    keeps the previous call's contents; every region a call reads it writes first, so nothing
+ *    needs clearing. */
+#define BFLY_STATIC_MAX_SAMPLES 65536
+int bfly_correlate_static(const bfly_bank *bank, const float *x_dev, int64_t n_samples,
+                          int64_t lag_begin, int64_t lag_end, float *rho_max_dev,
+                          int32_t *arg_lag_dev, void *stream);
+
 /* The same with an explicit correlation form (BFLY_FORM_*). */
 int bfly_correlate_form(const bfly_bank *bank, int form, const float *x_dev, int64_t n_samples,
                         int64_t lag_begin, int64_t lag_end,

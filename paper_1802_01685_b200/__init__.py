@@ -60,6 +60,7 @@ def _load():
     lib.bfly_bank_reserve.argtypes = [vp, i64]
     lib.bfly_correlate.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
     lib.bfly_correlate_form.argtypes = [vp, C.c_int, vp, i64, i64, i64, vp, vp, vp]
+    lib.bfly_correlate_static.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
     lib.bfly_correlate_multi.argtypes = [vp, i32, vp, i64, i64, i64, vp, vp, vp]
     lib.bfly_butterfly_map.argtypes = [vp, vp, vp, f32, i64, i32, f64, f64, i32, i32, vp, vp, vp]
     lib.bfly_tails.argtypes = [vp, vp, i64, i64, i64, f32, vp, i64, vp, vp, vp, vp, vp]
@@ -77,7 +78,7 @@ def _load():
     lib.bfly_launch_count.argtypes = []
     lib.bfly_launch_count.restype = i64
     for name in ("bfly_make_bank", "bfly_make_bank_grid", "bfly_bank_get", "bfly_bank_reserve",
-                 "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_correlate_multi", "bfly_butterfly_map",
+                 "bfly_bank_set_timing", "bfly_bank_core_ms", "bfly_correlate", "bfly_correlate_form", "bfly_correlate_multi", "bfly_correlate_static", "bfly_butterfly_map",
                  "bfly_search_host", "bfly_debug_fft_tc", "bfly_debug_fft_tc5", "bfly_tails", "bfly_hits_map",
                  "bfly_time_randomize", "bfly_coincidence", "bfly_pseudo_spectrum",
                  "bfly_make_bank3", "bfly_bank_get_f2", "bfly_debug_peak", "bfly_make_bank_settle",
@@ -244,6 +245,22 @@ def correlate_form(bank: Bank, form: int, x: torch.Tensor, lag_begin: int = 0,
 def correlate(bank: Bank, x: torch.Tensor, lag_begin: int = 0, lag_end: int | None = None,
               rho_max: torch.Tensor | None = None, arg_lag: torch.Tensor | None = None):
     return correlate_form(bank, FORM_DEFAULT, x, lag_begin, lag_end, rho_max, arg_lag)
+
+
+STATIC_MAX_SAMPLES = 65536        # BFLY_STATIC_MAX_SAMPLES (include/bfly.h)
+
+
+def correlate_static(bank: Bank, x: torch.Tensor, rho_max: torch.Tensor, arg_lag: torch.Tensor,
+                     lag_begin: int = 0, lag_end: int | None = None):
+    """bfly_correlate_static on torch's current stream: the default form with its scratch in a
+    static device array (no allocation inside the library); the caller passes the outputs."""
+    T, n = len(bank), x.numel()
+    lag_end = n - bank.L + 1 if lag_end is None else lag_end
+    _check(_lib.bfly_correlate_static(bank._h, _dev(x, torch.float32, "x", bank.device), n, int(lag_begin),
+                                      int(lag_end), _dev(rho_max, torch.float32, "rho_max", bank.device, T),
+                                      _dev(arg_lag, torch.int32, "arg_lag", bank.device, T),
+                                      _stream(bank.device)), "bfly_correlate_static")
+    return rho_max, arg_lag
 
 
 def correlate_multi(bank: Bank, xs, lag_begin: int = 0, lag_end: int | None = None):

@@ -613,6 +613,25 @@ int bfly_correlate(const bfly_bank *bank, const float *x_dev, int64_t n_samples,
                                rho_max_dev, arg_lag_dev, stream);
 }
 
+// The default form with its scratch in a static device array: allocates nothing (no cudaMalloc, no
+// cudaFree, no allocating library call), touches no state of the bank, takes no bank lock.
+int bfly_correlate_static(const bfly_bank *bank, const float *x_dev, int64_t n_samples, int64_t lag_begin,
+                          int64_t lag_end, float *rho_max_dev, int32_t *arg_lag_dev, void *stream)
+{
+    int form = BFLY_FORM_FFT_TC;
+    int rc = correlate_check(bank, &form, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev);
+    if (rc) return rc;
+    if (n_samples > BFLY_STATIC_MAX_SAMPLES) {
+        set_error("bfly_correlate_static: n_samples = %lld exceeds BFLY_STATIC_MAX_SAMPLES = %d (the static scratch "
+                  "array holds one segment of that size; use bfly_correlate)", (long long)n_samples,
+                  (int)BFLY_STATIC_MAX_SAMPLES);
+        return BFLY_ERANGE;
+    }
+    BFLY_ENTER(bank);
+    return launch_fft_tc_static(bank, x_dev, n_samples, lag_begin, lag_end, rho_max_dev, arg_lag_dev,
+                                (cudaStream_t)stream);
+}
+
 int bfly_butterfly_map(const bfly_bank *bank, const float *rho_max_dev, const int32_t *arg_lag_dev,
                        float kappa, int64_t lag_origin, int32_t samples_per_tbin, double f_lo_hz,
                        double df_hz, int32_t n_fbins, int32_t n_tbins, uint32_t *map_dev,

@@ -1029,6 +1029,70 @@ int launch_tails_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64
     return launch_tc_common(b, 1, &x, n_samples, lag_begin, lag_end, nullptr, nullptr, &ta, stream);
 }
 
+// ------------------------------------------------------------------------------------------
+// bfly_correlate_static: the default form with its per-call scratch (data-block spectra, per-lag
+// normalisers, block scales) in a file-scope device array instead of the bank's cudaMalloc'ed
+// workspace, for callers that must not allocate (CUDA graph capture, serving loops).  The array is
+// sized for one segment of BFLY_STATIC_MAX_SAMPLES samples (16 overlap-save blocks); every GPU
+// that loads the library holds it until exit.  All calls share it: calls that overlap on the GPU
+// race.  Nothing in it has to start at zero -- every region the kernels read is written first by
+// the same call (spectra and scales by tc_spectra_kernel, normalisers by tc_norm_kernel and
+// sliding_norm_kernel) -- so the previous call's contents are simply overwritten.
+constexpr int64_t STATIC_MAX_BLOCKS = BFLY_STATIC_MAX_SAMPLES / TCV;                       // 16
+constexpr size_t ST_OFF_XH = 0;                                                             // 16 x 32 KB, fp16
+constexpr size_t ST_OFF_RN2P = ST_OFF_XH + (size_t)STATIC_MAX_BLOCKS * 2 * EXCH_WORDS * 2;  // 16 x 16 KB, fp32
+constexpr size_t ST_OFF_RN2 = ST_OFF_RN2P + (size_t)STATIC_MAX_BLOCKS * TCV * 4;            // 64 Ki lags, fp32
+constexpr size_t ST_OFF_QS = ST_OFF_RN2 + (size_t)BFLY_STATIC_MAX_SAMPLES * 4;              // 16 doubles
+constexpr size_t ST_BYTES = ST_OFF_QS + 256;
+static __device__ __align__(256) unsigned char tc_static_scratch[ST_BYTES];                // 1 MB + 256 B
+
+// In host code `tc_static_scratch` is a host-side stand-in, not a device address: the address the
+// kernels get comes from cudaGetSymbolAddress, asked once per device with that device current.
+static int tc_static_base(int device, unsigned char **base)
+{
+    static PerDeviceOnce once;
+    static unsigned char *ptr[MAX_DEVICES] = {};
+    const int rc = once.run(device, [device]() -> int {
+        void *p = nullptr;
+        BFLY_CUDA(cudaGetSymbolAddress(&p, tc_static_scratch));
+        ptr[device] = static_cast<unsigned char *>(p);
+        return BFLY_OK;
+    });
+    if (rc) return rc;
+    *base = ptr[device];
+    return BFLY_OK;
+}
+
+int launch_fft_tc_static(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin, int64_t lag_end,
+                         float *rho_max, int32_t *arg_lag, cudaStream_t stream)
+{
+    const int64_t n_lags = lag_end - lag_begin;
+    int64_t n_blocks; int32_t n_tail;
+    tc_plan(n_lags, &n_blocks, &n_tail);
+    if (n_samples > BFLY_STATIC_MAX_SAMPLES || n_lags > BFLY_STATIC_MAX_SAMPLES || n_blocks > STATIC_MAX_BLOCKS) {
+        set_error("bfly_correlate_static: n_samples = %lld exceeds BFLY_STATIC_MAX_SAMPLES = %d (the static scratch "
+                  "array holds one segment of that size; use bfly_correlate)", (long long)n_samples,
+                  (int)BFLY_STATIC_MAX_SAMPLES);
+        return BFLY_ERANGE;
+    }
+    unsigned char *base = nullptr;
+    int rc = tc_static_base(b->device, &base);
+    if (rc) return rc;
+    // a host-side view of the bank whose workspace is the static array (the bank itself is not touched)
+    bfly_bank view = *b;
+    view.xh = reinterpret_cast<__half *>(base + ST_OFF_XH);
+    view.xh_cap = STATIC_MAX_BLOCKS * 2 * EXCH_WORDS;
+    view.rn2p = reinterpret_cast<float *>(base + ST_OFF_RN2P);
+    view.rn2p_cap = STATIC_MAX_BLOCKS * TCV;
+    view.rn2 = reinterpret_cast<float *>(base + ST_OFF_RN2);
+    view.rn2_cap = BFLY_STATIC_MAX_SAMPLES;
+    view.qs = reinterpret_cast<double *>(base + ST_OFF_QS);
+    view.qs_cap = STATIC_MAX_BLOCKS;
+    view.timing = 0;
+    if ((rc = launch_sliding_norm(x, n_samples, view.L, lag_begin, n_lags, view.rn2, stream))) return rc;
+    return launch_tc_common(&view, 1, &x, n_samples, lag_begin, lag_end, &rho_max, &arg_lag, nullptr, stream);
+}
+
 int launch_debug_fft_tc(const float2 *y, float2 *z, int full, cudaStream_t stream)
 {
     int dev = 0;

@@ -166,6 +166,8 @@ int launch_map(const bfly_bank *b, const float *rho_max, const int32_t *arg_lag,
 int64_t fft_blocks_needed(int32_t L, int64_t n_lags);
 int launch_fft_tc(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin,
                   int64_t lag_end, float *rho_max, int32_t *arg_lag, cudaStream_t stream);
+int launch_fft_tc_static(const bfly_bank *b, const float *x, int64_t n_samples, int64_t lag_begin, int64_t lag_end,
+                         float *rho_max, int32_t *arg_lag, cudaStream_t stream);
 int64_t tc_blocks_needed(int64_t n_lags);
 bool tc_multi_supported(int32_t L, int64_t n_lags);
 int launch_fft_tc_multi(const bfly_bank *b, int n_seg, const float *const *x, int64_t n_samples, int64_t lag_begin,
