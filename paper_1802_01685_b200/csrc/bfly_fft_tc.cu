@@ -241,6 +241,14 @@ __device__ __forceinline__ void synth_sincos(uint32_t Ahi, uint32_t Alo, uint32_
 // differ in bits 0-4, of which the folds keep bits 0-2 a permutation: still conflict free.
 __device__ __forceinline__ int gs_slot(int th) { return th ^ ((th >> 2) & 2) ^ ((th >> 4) & 1); }
 
+// (q & m8) | rank as ONE lop3 (LUT 0xEA = (a & b) | c); the compiler left to itself emits two
+__device__ __forceinline__ float rank_key(float q, uint32_t m8, uint32_t rank)
+{
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(__float_as_uint(q)), "r"(m8), "r"(rank));
+    return __uint_as_float(r);
+}
+
 // Index of tail-window sample n in sm.xt: a thread's lanes differ in bits 7-9 (g) and 11-12 (t)
 // of n; folding those into the bank bits makes the reads conflict free.
 __device__ __forceinline__ int xt_slot(int n) { return n ^ ((n >> 7) & 7) ^ (((n >> 11) & 3) << 3); }
@@ -389,6 +397,8 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                       sm.bar + 3 + (int)issued);
             next_b = next_b + 1 == seq_blocks ? 0 : next_b + 1;
         }
+    uint32_t m8 = 0xFFFFFFF8u;                         // in a register, so that (q & m8) | rank is one LOP3
+    asm volatile("" : "+r"(m8));
     int gs_tid = gs_slot(tid);                         // held in a register: recomputing it costs the block loop two instructions
     asm volatile("" : "+r"(gs_tid));
     uint32_t xcnt = 0;                                 // blocks consumed: slot = xcnt & 1, parity = (xcnt >> 1) & 1
@@ -660,8 +670,15 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
         const float4 *rn2p_s = MULTI ? rn2p + (int64_t)sg * n_blocks * (NT * 2) : rn2p;
         const float *rn2_s = MULTI ? sa.rn2[sg] : rn2;
         const float4 *rp_run = rn2p_s + tid * 2;       // MULTI: this thread's normalisers, block by block
-        float best = -1.0f;
-        int32_t code = 0;                              // 8 b + 4 e + i
+        // A7 inside the thread: the low three mantissa bits of q (2^-21 relative, far below the fp16
+        // operand noise) are replaced by 7 - rank, rank = 4 e + i the order of the lag among the
+        // thread's eight lags of a block (lag = .. + i + 64 e): the largest key is the largest q and,
+        // on a tie, the smallest lag (reading C8) -- one LOP3 per lag and a tree of three-input
+        // maxima instead of a compare, a select and an index update per lag (-9 instructions per
+        // block).  bcmp = bkey with its low bits at 7, so that a later block wins only with a larger
+        // q.  NaN keys (0 x -inf, or -inf with rank bits: lags past the last one) never win a maximum.
+        float bkey = -1.0f, bcmp = -1.0f;
+        int32_t bblk = 0;
         if (n_blocks > 0) front();
         for (int32_t b = 0; b < n_blocks; ++b) {
             mbar_wait(sm.bar + rb, (fpar >> rb) & 1);
@@ -704,17 +721,15 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                         qs4[i] = q;
                         qmax = fmaxf(qmax, fmaxf(q.x, q.y));
                     } else {
-                        // A7 inside the thread, in lag order (reading C8: ties to the smallest lag): the
-                        // thread's lags of this block are .. + i + 64 e, so the e = 0 lags are compared
-                        // here and the e = 1 lags after the loop; code = 8 b + 4 e + i
-                        if (q.x > best) { best = q.x; code = 8 * b + i; }
-                        qs4[i].y = q.y;
+                        qs4[i].x = rank_key(q.x, m8, 7u - i);
+                        qs4[i].y = rank_key(q.y, m8, 3u - i);
                     }
                 }
                 if (!TAILS) {
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-                        if (qs4[i].y > best) { best = qs4[i].y; code = 8 * b + 4 + i; }
+                    const float bm = fmaxf(fmaxf(fmaxf(qs4[0].x, qs4[1].x), qs4[2].x),
+                                           fmaxf(fmaxf(fmaxf(qs4[3].x, qs4[0].y), qs4[1].y),
+                                                 fmaxf(fmaxf(qs4[2].y, qs4[3].y), -1.0f)));
+                    if (bm > bcmp) { bkey = bm; bcmp = __uint_as_float(__float_as_uint(bm) | 7u); bblk = b; }
                 }
                 if (TAILS && qmax > thr) {                 // rare: at least one of this thread's 8 lags is a hit
 #pragma unroll
@@ -766,7 +781,8 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                         }
                     } else {
                         const float q = m2 * __ldg(rn2_s + (int64_t)n_blocks * TCV + r);
-                        if (q > best) { best = q; code = 8 * n_blocks + r; }
+                        const float kq = rank_key(q, m8, 7u - (uint32_t)r);
+                        if (kq > bcmp) { bkey = kq; bcmp = __uint_as_float(__float_as_uint(kq) | 7u); bblk = n_blocks; }
                     }
                 }
             }
@@ -791,14 +807,16 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                 }
             } else {
                 const float q = fmaf(s, s, c * c) * __ldg(rn2_s + (int64_t)n_blocks * TCV + tid);
-                if (q > best) { best = q; code = 8 * n_blocks + tid; }
+                const float kq = rank_key(q, m8, 7u - (uint32_t)tid);
+                if (kq > bcmp) { bkey = kq; bcmp = __uint_as_float(__float_as_uint(kq) | 7u); bblk = n_blocks; }
             }
         }
         if (!TAILS) {
             unsigned long long p = 0ull;
+            const float best = __uint_as_float(__float_as_uint(bkey) & 0xFFFFFFF8u);
             if (best > 0.0f) {                         // q = 0 everywhere: rho = 0 at the first lag (write_out)
-                const int bb = code >> 3, rank = code & 7;            // rank = 4 e + i
-                const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * TCV + (uint32_t)(code - 8 * n_blocks)
+                const int bb = bblk, rank = 7 - (int)(__float_as_uint(bkey) & 7u);   // rank = 4 e + i (tail lags: r)
+                const uint32_t li = bb >= n_blocks ? (uint32_t)n_blocks * TCV + (uint32_t)rank
                                                    : (uint32_t)bb * TCV + (uint32_t)((4 * w + (rank & 3)) +
                                                                                      64 * (2 * t + (rank >> 2)) + 512 * g);
                 p = ((unsigned long long)__float_as_uint(best) << 32) | (unsigned long long)(0xFFFFFFFFu - li);
