@@ -168,7 +168,9 @@ __global__ void dense_prep_kernel(const float *__restrict__ x, int64_t n_samples
     }
     if (idx < n_lags_padded) {
         const float inv = 1.0f / sc;      // a power of two: the products below are exact
-        rn2s[idx] = idx < n_lags ? __ldg(rn2 + idx) * inv * inv : 0.0f;
+        // stored in the order the epilogue reads it: lag 8 r + s of a 256-lag tile at s * 32 + r
+        const int64_t e = (idx & ~(int64_t)255) + (idx & 7) * 32 + ((idx & 255) >> 3);
+        rn2s[e] = idx < n_lags ? __ldg(rn2 + idx) * inv * inv : 0.0f;
     }
 }
 
@@ -221,6 +223,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, 
         uint32_t phase = 0, tiles_done = 0;
         const int row = tid & (DT_M - 1), half = tid >> 7;
         const uint32_t row_off = (uint32_t)row * 128u, row_x = (uint32_t)row & 7u;
+        uint32_t m32 = 0xFFFFFFE0u;                // in a register: (q & m32) | rank is then one LOP3
+        asm volatile("" : "+r"(m32));
         unsigned long long *merge = reinterpret_cast<unsigned long long *>(dt_raw + (sbase - saddr(dt_raw)) +
                                                                           DT_STAGES * DT_STAGE_BYTES + 128);
         for (int64_t tt = blockIdx.x; tt < n_ttiles; tt += gridDim.x) {
@@ -232,7 +236,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, 
             // angle (|f1| / fs^2 cycles): two terms of the series are exact in fp32
             const float wx = (float)(long long)(2ull * Bq) * 3.4061215800865545e-19f;   // 2 pi 2^-64
             const float wr = fmaf(-0.5f * wx, wx, 1.0f), wi = fmaf(wx * wx * (-1.0f / 6.0f), wx, wx);
-            unsigned long long best = 0ull;
+            float bkey = -1.0f, bcmp = -1.0f;      // running key of this thread's columns, and the same with its rank bits set
+            int32_t bchunk = 0;                    // 8 lt + s of the chunk that holds it
             for (int32_t lt = 0; lt < n_lag_tiles; ++lt) {
                 for (int32_t kb = 0; kb < n_kb; ++kb) {
                     bar_wait(empty(stage), phase ^ 1u);
@@ -344,7 +349,12 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, 
                     bar_arrive(full(stage));
                     if (++stage == DT_STAGES) { stage = 0; phase ^= 1u; }
                 }
-                // ---- epilogue of this lag tile: column s * 32 + r holds lag 8 r + s of the tile
+                // ---- epilogue of this lag tile: column s * 32 + r holds lag 8 r + s of the tile.  A7 per
+                //      thread by rank-in-mantissa keys: the low five mantissa bits of q (2^-18 relative)
+                //      are replaced by 31 - r, so that the maximum key of a 32-column chunk is its largest
+                //      q and, on a tie, its smallest lag; chunks are compared by one test each (the tie of
+                //      two chunks is resolved on the lags themselves).  Lags past the last one carry a
+                //      normaliser of 0 (q = 0: they never beat a positive q).
                 bar_wait(tmem_full, tiles_done & 1u);
                 tc_fence_after();
                 const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
@@ -354,22 +364,46 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap xmap, int64_t T, int32_t L, 
                     tmem_ld32(lane_addr + (uint32_t)(s * 32), vc);
                     tmem_ld32(lane_addr + (uint32_t)(DT_N + s * 32), vs);
                     tmem_ld_wait();
-                    const int64_t lag0 = (int64_t)lt * DT_N + s;
+                    if (s == 4 * half + 3) {           // the accumulators are in registers: the next tile's MMAs may start
+                        tc_fence_before();
+                        bar_arrive(tmem_empty);
+                    }
+                    const float4 *rp = reinterpret_cast<const float4 *>(rn2s + ((int64_t)lt * DT_N + s * 32));
+                    float m[4] = {-1.0f, -1.0f, -1.0f, -1.0f};
 #pragma unroll
-                    for (int r = 0; r < 32; ++r) {
-                        const int64_t li = lag0 + 8 * r;
-                        if (li < n_lags) {
+                    for (int r4 = 0; r4 < 8; ++r4) {
+                        const float4 rv = __ldg(rp + r4);
+                        const float rr[4] = {rv.x, rv.y, rv.z, rv.w};
+#pragma unroll
+                        for (int kq = 0; kq < 4; ++kq) {
+                            const int r = 4 * r4 + kq;
                             const float c = __uint_as_float(vc[r]), sq = __uint_as_float(vs[r]);
-                            const float q = fmaf(sq * sq, is, c * c * ic) * __ldg(rn2s + li);
-                            const unsigned long long key =
-                                ((unsigned long long)__float_as_uint(q) << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)li);
-                            if (q > 0.0f && key > best) best = key;
+                            const float q = fmaf(sq * sq, is, c * c * ic) * rr[kq];
+                            uint32_t key;
+                            asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(key) : "r"(__float_as_uint(q)), "r"(m32), "r"(31u - r));
+                            m[kq] = fmaxf(m[kq], __uint_as_float(key));
                         }
                     }
+                    const float bm = fmaxf(fmaxf(m[0], m[1]), fmaxf(m[2], m[3]));
+                    const uint32_t bmu = __float_as_uint(bm);
+                    const int32_t chunk = lt * 8 + s;
+                    if (bm > bcmp) {
+                        bkey = bm; bcmp = __uint_as_float(bmu | 31u); bchunk = chunk;
+                    } else if ((bmu | 31u) == __float_as_uint(bcmp)) {      // equal q: the smaller lag (rare)
+                        const int32_t l_new = (chunk >> 3) * DT_N + 8 * (31 - (int32_t)(bmu & 31u)) + (chunk & 7);
+                        const int32_t l_old = (bchunk >> 3) * DT_N + 8 * (31 - (int32_t)(__float_as_uint(bkey) & 31u)) + (bchunk & 7);
+                        if (l_new < l_old) { bkey = bm; bchunk = chunk; }
+                    }
                 }
-                tc_fence_before();
-                bar_arrive(tmem_empty);
                 ++tiles_done;
+            }
+            unsigned long long best = 0ull;
+            {
+                const uint32_t ku = __float_as_uint(bkey), qbits = ku & 0xFFFFFFE0u;
+                if (__uint_as_float(qbits) > 0.0f) {
+                    const uint32_t li = (uint32_t)((bchunk >> 3) * DT_N + 8 * (31 - (int32_t)(ku & 31u)) + (bchunk & 7));
+                    best = ((unsigned long long)qbits << 32) | (unsigned long long)(0xFFFFFFFFu - li);
+                }
             }
             // the two column halves of a row meet in shared memory (the tile handshakes keep the
             // next tile's writes behind this tile's reads)
