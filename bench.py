@@ -166,6 +166,10 @@ def run_reference(args, cfg, rank):
     """--impl reference: the float64 oracle on the box's host cores (rank 0 only)."""
     if rank != 0:
         return
+    # the same process environment as the main arm's cpu_baseline leg, which runs after torch has
+    # been imported (round 1 measured the oracle 1.5x slower in a process without it: the OpenMP
+    # runtime behaves differently); torch does no work here
+    import torch  # noqa: F401
     import oracle
     x = make_data(cfg)
     f0a, f1a = bank_grid(cfg)
