@@ -562,7 +562,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     }
                 }
             }
-            chain1(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
+            chain1<TAILS>(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
         }
         __syncthreads();                                // every warp has left the previous template
         // (the per-template chores are spread over warps 0, 8 and 12 so that no warp trails the others
@@ -661,7 +661,7 @@ tc_correlate_kernel(int64_t T, int32_t L, const uint64_t *__restrict__ phA,
                     yi[2 * ci + h] = as_u32(__hfma2(xi, gr, __hmul2(xr, gi)));
                 }
             }
-            chain1(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
+            chain1<TAILS>(k, yr, yi, sm.exch + wb * (EXCH_WORDS / 4), tid);
             __syncwarp();
             if (lane == 0) mbar_arrive(sm.bar + wb);
             wb = wb + 1 == N_EXCH ? 0 : wb + 1;

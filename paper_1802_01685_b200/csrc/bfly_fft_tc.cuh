@@ -128,6 +128,7 @@ struct ConstsT {
     tw_t twAB;               // e = 0, 1: w_64^(g (2t+e)) / S8:            alpha = g, b = 2t + e
     tw_t twBig[8];           // [ci*2+h], e = 0, 1: w_8192^((2t+e + 8g)(16 c + d')) / S8
     tw_t twC[2];             // [h], e = 0, 1: w_128^((8h + 2t + e) g) / S8:  gamma = g
+    uint32_t st_off[4];      // [2 e + p]: byte offset of this thread's chunk (U = 2t + e + 8g, chunk0 + p) in an exchange buffer
 };
 
 // exp(+2 pi i num / den) * scale, num reduced mod den first (den a power of two <= 8192)
@@ -147,6 +148,12 @@ __device__ __forceinline__ void dft_frag(uint32_t (&a)[3], int r, float scale, i
     a[2] = pack_h2(-w0.y, -w1.y);
 }
 
+// Byte-free addressing of an exchange buffer, in 16-byte chunks: unit U = alpha + 8 beta owns 32
+// chunks; chunk (d' & 7) * 4 + (c >> 1) holds {Re(d'<8), Im(d'<8), Re(d'>=8), Im(d'>=8)} of the
+// c pair as four fp16x2 words.  The XOR makes both the stores (lanes differ in U) and the loads
+// (lanes differ in chunk) bank-conflict free.
+__device__ __forceinline__ int exch_chunk(int U, int chunk) { return U * 32 + (chunk ^ ((U >> 1) & 7)); }
+
 // Warp w handles, before the exchange, the eight 64-point sub-transforms ("units") with
 // c = 4 (w >> 3) + ci, d' = (w & 7) + 8 h  (unit index u = 2 ci + h), and after it the four
 // units with alpha + 8 beta = 4 w + i.
@@ -165,19 +172,27 @@ __device__ __forceinline__ void make_consts(ConstsT<HALF> &k, int tid)
         k.twBig[u] = make_tw<HALF>(root((2 * t + 8 * g) * (16 * c + dp), 8192, r8),
                                 root((2 * t + 1 + 8 * g) * (16 * c + dp), 8192, r8));
     }
+    {
+        const int chunk0 = (w & 7) * 4 + 2 * (w >> 3);
+#pragma unroll
+        for (int e = 0; e < 2; ++e)
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+                k.st_off[2 * e + p] = 16u * (uint32_t)exch_chunk(2 * t + e + 8 * g, chunk0 + p);
+                asm volatile("" : "+r"(k.st_off[2 * e + p]));      // held as byte offsets: STS [R + UR], no LEA per store
+            }
+    }
 #pragma unroll
     for (int h = 0; h < 2; ++h)
         k.twC[h] = make_tw<HALF>(root((8 * h + 2 * t) * g, 128, r8), root((8 * h + 2 * t + 1) * g, 128, r8));
 }
 
-// Byte-free addressing of an exchange buffer, in 16-byte chunks: unit U = alpha + 8 beta owns 32
-// chunks; chunk (d' & 7) * 4 + (c >> 1) holds {Re(d'<8), Im(d'<8), Re(d'>=8), Im(d'>=8)} of the
-// c pair as four fp16x2 words.  The XOR makes both the stores (lanes differ in U) and the loads
-// (lanes differ in chunk) bank-conflict free.
-__device__ __forceinline__ int exch_chunk(int U, int chunk) { return U * 32 + (chunk ^ ((U >> 1) & 7)); }
-
 // Passes A and B of the eight units of this warp.  In: yr[u], yi[u] = B fragments (fp16x2 pairs
 // over a = 2t, 2t+1; column b = g).  Out: stored to the exchange buffer.
+// BYTE_OFF: store through the precomputed byte offsets k.st_off (STS [R + UR], no LEA per store)
+// instead of chunk indices.  Measured at config 4: the max / argmax kernel is 0.3 % slower with
+// it, the kappa-sigma tails kernel (higher register pressure) 2.5 % faster: used there only.
+template <bool BYTE_OFF = false>
 __device__ __forceinline__ void chain1(const ConstsT<false> &k, const uint32_t (&yr)[8],
                                        const uint32_t (&yi)[8], uint4 *exch, int tid)
 {
@@ -203,11 +218,13 @@ __device__ __forceinline__ void chain1(const ConstsT<false> &k, const uint32_t (
             q.y = e ? pack_h2(v[4 * p].i.y, v[4 * p + 2].i.y) : pack_h2(v[4 * p].i.x, v[4 * p + 2].i.x);
             q.z = e ? pack_h2(v[4 * p + 1].r.y, v[4 * p + 3].r.y) : pack_h2(v[4 * p + 1].r.x, v[4 * p + 3].r.x);
             q.w = e ? pack_h2(v[4 * p + 1].i.y, v[4 * p + 3].i.y) : pack_h2(v[4 * p + 1].i.x, v[4 * p + 3].i.x);
-            exch[exch_chunk(U, chunk0 + p)] = q;
+            if (BYTE_OFF) *reinterpret_cast<uint4 *>(reinterpret_cast<unsigned char *>(exch) + k.st_off[2 * e + p]) = q;
+            else exch[exch_chunk(U, chunk0 + p)] = q;
         }
     }
 }
 
+template <bool BYTE_OFF = false>     // (ignored by the all-fp16 variant)
 __device__ __forceinline__ void chain1(const ConstsT<true> &k, const uint32_t (&yr)[8],
                                        const uint32_t (&yi)[8], uint4 *exch, int tid)
 {
